@@ -1,0 +1,276 @@
+"""CPU oracle, Python side.  TEST INFRASTRUCTURE ONLY (tests/, __graft_entry__.smoke(), bench.py cpu_baseline).
+
+* thin ctypes wrapper over oracle/ltjk_oracle.c (built on demand with gcc -O2 -fopenmp; no CUDA, no torch);
+* O7 contraction  J = einsum('mnkr,kr->mn'), K = einsum('mknr,kr->mn')            PAPER.md:L157 Eq. (17)
+* O9 minimax Laplace grid by Remez exchange + Newton in 120-digit arithmetic       PAPER.md:L126 Eq. (11)
+* O10 pseudo-density as explicit loops                                            PAPER.md:L136-145 Eqs. (13),(15)
+
+Nothing here imports the CUDA package except the shared, arithmetic-free input generators.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SO = _HERE / "libltjk_oracle.so"
+_SRC = _HERE / "ltjk_oracle.c"
+_lib = None
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_ip = ctypes.POINTER(ctypes.c_int)
+_lp = ctypes.POINTER(ctypes.c_longlong)
+
+
+def build(force: bool = False) -> Path:
+    """Compile the C oracle (building the checker is not using it)."""
+    if force or not _SO.exists() or _SO.stat().st_mtime < _SRC.stat().st_mtime:
+        cmd = ["gcc", "-O2", "-march=native", "-fopenmp", "-std=c11", "-shared", "-fPIC", "-o", str(_SO),
+               str(_SRC), "-lm"]
+        subprocess.check_call(cmd)
+    return _SO
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(str(_SO))
+        _lib.orc_jk_folded.restype = ctypes.c_longlong
+        _lib.orc_nao.restype = ctypes.c_int
+        _lib.orc_max_threads.restype = ctypes.c_int
+    return _lib
+
+
+def _d(a):
+    return a.ctypes.data_as(_dp)
+
+
+def _i(a):
+    return a.ctypes.data_as(_ip)
+
+
+def _basis_args(b):
+    xyz = np.ascontiguousarray(b.xyz, dtype=np.float64)
+    atom = np.ascontiguousarray(b.atom, dtype=np.int32)
+    l = np.ascontiguousarray(b.l, dtype=np.int32)
+    nprim = np.ascontiguousarray(b.nprim, dtype=np.int32)
+    poff = np.ascontiguousarray(b.prim_off, dtype=np.int32)
+    exps = np.ascontiguousarray(b.exps, dtype=np.float64)
+    coef = np.ascontiguousarray(b.coef, dtype=np.float64)
+    keep = (xyz, atom, l, nprim, poff, exps, coef)
+    args = (ctypes.c_int(xyz.shape[0]), _d(xyz), ctypes.c_int(l.shape[0]), _i(atom), _i(l), _i(nprim), _i(poff),
+            _d(exps), _d(coef))
+    return args, keep
+
+
+def max_threads() -> int:
+    return int(lib().orc_max_threads())
+
+
+def boys(mmax: int, T: float) -> np.ndarray:
+    F = np.zeros(mmax + 1)
+    lib().orc_boys(ctypes.c_int(mmax), ctypes.c_double(T), _d(F))
+    return F
+
+
+_NC = (1, 3, 6)
+
+
+def eri_shell(b, A, B, C, D) -> np.ndarray:
+    args, keep = _basis_args(b)
+    shp = tuple(_NC[int(b.l[s])] for s in (A, B, C, D))
+    out = np.zeros(shp)
+    lib().orc_eri_shell(*args, ctypes.c_int(A), ctypes.c_int(B), ctypes.c_int(C), ctypes.c_int(D), _d(out))
+    return out
+
+
+def eri_tensor(b) -> np.ndarray:
+    """O7: the full N^4 tensor, no symmetry used."""
+    args, keep = _basis_args(b)
+    n = b.nao
+    out = np.zeros((n, n, n, n))
+    lib().orc_eri_tensor(*args, _d(out))
+    return out
+
+
+def schwarz(b) -> np.ndarray:
+    args, keep = _basis_args(b)
+    Q = np.zeros((b.nshell, b.nshell))
+    lib().orc_schwarz(*args, _d(Q))
+    return Q
+
+
+def jk_definition(eri: np.ndarray, D: np.ndarray):
+    """O7 contraction, Eq. (17) literally.  D: [nD,N,N]."""
+    J = np.einsum("mnkr,dkr->dmn", eri, D, optimize=True)
+    K = np.einsum("mknr,dkr->dmn", eri, D, optimize=True)
+    return J, K
+
+
+def jk_folded(b, D: np.ndarray, tau: float, pair_range=None, Q=None):
+    """O6.  Returns J, K [nD,N,N] and the number of shell quartets kept."""
+    args, keep = _basis_args(b)
+    D = np.ascontiguousarray(D, dtype=np.float64)
+    nD, n, _ = D.shape
+    J = np.zeros_like(D)
+    K = np.zeros_like(D)
+    npair = b.nshell * (b.nshell + 1) // 2
+    p0, p1 = (0, npair) if pair_range is None else pair_range
+    Qp = _d(np.ascontiguousarray(Q)) if Q is not None else None
+    kept = lib().orc_jk_folded(*args, ctypes.c_double(tau), ctypes.c_int(nD), _d(D), _d(J), _d(K),
+                               ctypes.c_longlong(p0), ctypes.c_longlong(p1), Qp)
+    return J, K, int(kept)
+
+
+def jk_blocks(b, D: np.ndarray, tau: float, shell_pairs, Q=None):
+    """Eq. (17) for sampled ordered shell pairs (X,Y): returns lists of J and K blocks [nD,nx,ny]."""
+    args, keep = _basis_args(b)
+    D = np.ascontiguousarray(D, dtype=np.float64)
+    nD = D.shape[0]
+    X = np.asarray([p[0] for p in shell_pairs], dtype=np.int32)
+    Y = np.asarray([p[1] for p in shell_pairs], dtype=np.int32)
+    sizes = [nD * _NC[int(b.l[x])] * _NC[int(b.l[y])] for x, y in zip(X, Y)]
+    off = np.zeros(len(sizes) + 1, dtype=np.int64)
+    off[1:] = np.cumsum(sizes)
+    Jb = np.zeros(int(off[-1]))
+    Kb = np.zeros(int(off[-1]))
+    Qp = _d(np.ascontiguousarray(Q)) if Q is not None else None
+    lib().orc_jk_blocks(*args, ctypes.c_double(tau), ctypes.c_int(nD), _d(D), ctypes.c_int(len(X)), _i(X), _i(Y),
+                        off.ctypes.data_as(_lp), _d(Jb), _d(Kb), Qp)
+    Js, Ks = [], []
+    for k, (x, y) in enumerate(zip(X, Y)):
+        shp = (nD, _NC[int(b.l[x])], _NC[int(b.l[y])])
+        Js.append(Jb[off[k]:off[k + 1]].reshape(shp).copy())
+        Ks.append(Kb[off[k]:off[k + 1]].reshape(shp).copy())
+    return Js, Ks
+
+
+# ---------------------------------------------------------------------------------------------------------
+# O10 pseudo-density, explicit loops (Eqs. (13), (15)):  D^{alpha,d}_{mu nu} =
+#     sum_{ia} C_{mu i} e^{+eps_i tau_alpha} T^d_{ia} e^{-eps_a tau_alpha} C_{nu a}
+# Output layout [ntau][nT][N][N].  No w_alpha, no 1/2, no spin factor (reading A10).
+def pseudo_densities_loops(C_occ, C_vir, eps_occ, eps_vir, T, tau) -> np.ndarray:
+    n, nocc = C_occ.shape
+    nvir = C_vir.shape[1]
+    nT = T.shape[0]
+    out = np.zeros((len(tau), nT, n, n))
+    for al, t in enumerate(tau):
+        for d in range(nT):
+            for i in range(nocc):
+                u = C_occ[:, i] * np.exp(eps_occ[i] * t)          # U~_{mu i}, Eq. (13)
+                for a in range(nvir):
+                    v = C_vir[:, a] * np.exp(-eps_vir[a] * t)     # V~_{nu a}, Eq. (13)
+                    out[al, d] += T[d, i, a] * np.outer(u, v)     # Eq. (15)
+    return out
+
+
+# ---------------------------------------------------------------------------------------------------------
+# O9 minimax exponential-sum approximation of 1/x on [xmin, xmax] (Eq. (11), refs 18-19 of the paper):
+# minimise max_x |1/x - sum_a w_a exp(-x tau_a)|.  Solved on [1, R], R = xmax/xmin, then tau = tau^/xmin,
+# w = w^/xmin.  Remez exchange on the 2k+1 alternation points with Newton on the 2k parameters + level,
+# started from the trapezoid rule for 1/x = int exp(-x e^s) e^s ds; 120-digit arithmetic (mpmath) so that the
+# oracle's grid is converged far beyond fp64.
+def laplace_minimax(xmin: float, xmax: float, k: int, verbose: bool = False):
+    import mpmath as mp
+    mp.mp.dps = 120   # the Newton matrices are very ill-conditioned: pivots far below 1e-50 occur
+    R = mp.mpf(xmax) / mp.mpf(xmin)
+
+    def err(x, tau, w):
+        return 1 / x - sum(wi * mp.e ** (-x * ti) for ti, wi in zip(tau, w))
+
+    def derr(x, tau, w):
+        return -1 / x ** 2 + sum(wi * ti * mp.e ** (-x * ti) for ti, wi in zip(tau, w))
+
+    def remez(Rc, tau, w, xs, iters=60):
+        delta = mp.mpf(0)
+        for it in range(iters):
+            # Newton on E(x_j) - (-1)^j delta = 0 for the unknowns (tau, w, delta)
+            for nit in range(60):
+                Fv = mp.matrix(2 * k + 1, 1)
+                Jm = mp.matrix(2 * k + 1, 2 * k + 1)
+                for j, x in enumerate(xs):
+                    Fv[j] = err(x, tau, w) - (-1) ** j * delta
+                    for a in range(k):
+                        ex = mp.e ** (-x * tau[a])
+                        Jm[j, a] = w[a] * x * ex
+                        Jm[j, k + a] = -ex
+                    Jm[j, 2 * k] = -(-1) ** j
+                dx = mp.lu_solve(Jm, -Fv)
+                # damped Newton: no parameter may change by more than 30 % in one step (keeps them positive)
+                rel = max(max(abs(dx[a] / tau[a]), abs(dx[k + a] / w[a])) for a in range(k))
+                step = min(mp.mpf(1), mp.mpf("0.3") / rel) if rel > 0 else mp.mpf(1)
+                tau = [tau[a] + step * dx[a] for a in range(k)]
+                w = [w[a] + step * dx[k + a] for a in range(k)]
+                delta = delta + step * dx[2 * k]
+                if max(abs(v) for v in dx) < mp.mpf(10) ** (-40):
+                    break
+            # exchange: move every interior point to the local extremum of E next to it; endpoints stay
+            new = [mp.mpf(1)]
+            for j in range(1, 2 * k):
+                lo, hi = xs[j - 1], xs[j + 1]
+                grid = [lo + (hi - lo) * t / 40 for t in range(41)]
+                sgn = mp.sign(err(xs[j], tau, w))
+                vals = [err(x, tau, w) * sgn for x in grid]
+                m = max(range(41), key=lambda t: vals[t])
+                a_, b_ = grid[max(m - 1, 0)], grid[min(m + 1, 40)]
+                try:
+                    xr = mp.findroot(lambda x: derr(x, tau, w), (a_, b_), solver="illinois",
+                                     tol=mp.mpf(10) ** (-40))
+                    if not (a_ <= xr <= b_):
+                        xr = grid[m]
+                except Exception:
+                    xr = grid[m]
+                new.append(xr)
+            new.append(Rc)
+            shift = max(abs(a - b) for a, b in zip(new, xs))
+            xs = new
+            if verbose:
+                print("remez R=%s it=%d delta=%s shift=%s" % (mp.nstr(Rc, 6), it, mp.nstr(delta, 8), mp.nstr(shift, 5)))
+            if shift < mp.mpf(10) ** (-25):
+                break
+        return tau, w, delta, xs
+
+    # Start: on a WIDER interval [1, R0] (well conditioned in fp64) fit by variable-projection least squares
+    # from the trapezoid rule for 1/x = int exp(-x e^s) e^s ds (library routines as steps), then walk R0 -> R
+    # in geometric steps, each a full Remez solve started from the previous one.
+    from scipy.optimize import least_squares
+    R0 = max(float(R), 10.0 ** (k / 3.0))
+    hh = (np.log(R0) + 5.5) / k
+    t0 = np.exp(-np.log(R0) - 2.5 + hh * (np.arange(k) + 0.5))
+    xg = np.exp(np.linspace(0.0, np.log(R0), 600))
+
+    def solve_w(lt):
+        A = np.exp(-xg[:, None] * np.exp(lt)[None, :])
+        ww, *_ = np.linalg.lstsq(A, 1.0 / xg, rcond=None)
+        return A, ww
+
+    sol = least_squares(lambda lt: solve_w(lt)[0] @ solve_w(lt)[1] - 1.0 / xg, np.log(t0), method="trf",
+                        xtol=1e-15, ftol=1e-15, gtol=1e-15, max_nfev=5000)
+    _, w0 = solve_w(sol.x)
+    order = np.argsort(sol.x)
+    tau = [mp.mpf(float(v)) for v in np.exp(sol.x[order])]
+    w = [mp.mpf(float(v)) for v in w0[order]]
+    if min(w) <= 0:
+        raise RuntimeError("laplace_minimax: least-squares start has a non-positive weight")
+    Rc = mp.mpf(R0)
+    xs = [Rc ** ((1 - mp.cos(mp.pi * j / (2 * k))) / 2) for j in range(2 * k + 1)]
+    tau, w, delta, xs = remez(Rc, tau, w, xs)
+    while Rc > R:
+        Rn = max(R, Rc / mp.mpf("1.3"))
+        xs = [Rn ** (mp.log(x) / mp.log(Rc)) for x in xs]
+        Rc = Rn
+        tau, w, delta, xs = remez(Rc, tau, w, xs)
+    xm = mp.mpf(xmin)
+    tau_o = np.array([float(t / xm) for t in tau])
+    w_o = np.array([float(x / xm) for x in w])
+    return tau_o, w_o, float(abs(delta) / xm), np.array([float(x * xm) for x in xs])
+
+
+def laplace_error_curve(tau, w, x):
+    x = np.asarray(x, dtype=np.float64)
+    return 1.0 / x - (np.asarray(w)[None, :] * np.exp(-x[:, None] * np.asarray(tau)[None, :])).sum(1)
