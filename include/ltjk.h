@@ -1,0 +1,128 @@
+/*
+ * ltjk.h -- C ABI of the B200-native non-symmetric Laplace-transform J/K build.
+ *
+ * The path (cited against /root/reference/PAPER.md as PAPER.md:L<n>):
+ *   basis upload -> shell pairs + Schwarz bounds -> minimax Laplace grid (Eq. 11)
+ *   -> pseudo-densities D^{alpha,d} = (C_o e^{+eps_o tau}) T_d (C_v e^{-eps_v tau})^T (Eqs. 13-15)
+ *   -> J[D], K[D] for a batch of general (non-symmetric) AO densities (Eq. 17; scatter rule Eq. 25)
+ *
+ * Conventions
+ *   - Every function returns 0 (LTJK_OK) or a negative LTJK_E* code; nothing throws or aborts across the ABI.
+ *     ltjk_last_error(ctx) gives a human-readable message for the last failure on that context.
+ *   - "host" pointers are ordinary CPU memory; "device" pointers are CUDA device memory on the context's
+ *     device (e.g. torch tensors' data_ptr()).  The library never frees caller memory and never returns
+ *     memory the caller must free.  Internal device buffers belong to the context.
+ *   - All device work is enqueued on the context's stream; calls that launch kernels return without
+ *     synchronising (the caller syncs through its own stream API) unless stated otherwise.
+ *   - A context is not thread-safe.
+ *   - There is NO CPU fallback: without a CUDA device ltjk_create fails with LTJK_ECUDA.
+ *   - Units: bohr, hartree (PAPER.md reports E_h/a_0 throughout, e.g. L450).
+ *   - No prefactor is embedded anywhere: no w_alpha, no exchange 1/2, no spin factor 2
+ *     ("J^x and K^x denote the single bare builds ... carry no embedded prefactor").
+ */
+#ifndef LTJK_H
+#define LTJK_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LTJK_OK        0
+#define LTJK_EINVAL   -1   /* bad argument (null pointer, negative size, nprim too large, ...) */
+#define LTJK_ENOBASIS -2   /* call order: basis / shell pairs not set yet */
+#define LTJK_ECUDA    -3   /* CUDA runtime error or no device */
+#define LTJK_ELMAX    -4   /* angular momentum > 2 (kernels are Cartesian s, p, d) */
+#define LTJK_ENOCONV  -5   /* Laplace quadrature did not converge (no silent fallback grid) */
+#define LTJK_ENOMEM   -6   /* device allocation failed */
+
+typedef struct ltjk_ctx ltjk_ctx;   /* opaque; owns all internal device buffers */
+
+/* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (e.g. torch's current stream
+ * handle) or NULL for the legacy default stream. */
+int ltjk_create(ltjk_ctx** out, int device, void* cuda_stream);
+int ltjk_destroy(ltjk_ctx* ctx);
+const char* ltjk_last_error(const ltjk_ctx* ctx);
+
+/* Upper bound, in bytes, on the integral-panel scratch the context may allocate (default 32 GiB, clamped to
+ * 60 % of free device memory at build_shell_pairs time).  Must be called before ltjk_build_shell_pairs. */
+int ltjk_set_scratch_bytes(ltjk_ctx* ctx, long long bytes);
+
+/* Basis upload (step a1).  HOST pointers, copied.
+ *   xyz[natom*3]        centres, bohr
+ *   atom[nshell]        centre index of each shell
+ *   l[nshell]           angular momentum, 0..2 (else LTJK_ELMAX)
+ *   nprim[nshell]       primitives per shell, 1..4
+ *   prim_off[nshell]    first primitive of the shell in exps/coef
+ *   exps[], coef[]      primitive exponents and coefficients.  coef multiplies
+ *                       (x-Ax)^i (y-Ay)^j (z-Az)^k exp(-a r^2) DIRECTLY: normalisation is the caller's job and
+ *                       is common to all Cartesian components of a shell (reading A6).
+ * AO order = shell order; Cartesian components lexicographic: p = x,y,z; d = xx,xy,xz,yy,yz,zz (reading A7).
+ * Kernels are Cartesian only. */
+int ltjk_set_basis(ltjk_ctx* ctx, int natom, const double* xyz, int nshell, const int* atom, const int* l,
+                   const int* nprim, const int* prim_off, const double* exps, const double* coef);
+int ltjk_get_nao(const ltjk_ctx* ctx, int* nao);
+
+/* Shell-pair builder (steps a2, a5).  For every shell pair: Gaussian-product data per primitive pair
+ * (p, P, PA, K_ab = c_a c_b exp(-ab/p R_AB^2)) and the Schwarz bound Q_AB = sqrt(max |(ab|ab)|)
+ * (PAPER.md:L176, L446), then the screened work lists: a shell quartet (AB|CD) is dropped iff
+ * Q_AB * Q_CD < schwarz_tau (pure integral Schwarz, no density weighting; reading A9).
+ * Synchronises.  Outputs (host, may be NULL):
+ *   n_pairs          number of canonical shell pairs A>=B
+ *   n_quartets_kept  number of canonical quartets (AB)>=(CD) with Q_AB Q_CD >= tau (8-fold unique count) */
+int ltjk_build_shell_pairs(ltjk_ctx* ctx, double schwarz_tau, long long* n_pairs, long long* n_quartets_kept);
+
+/* Copy the Schwarz bounds to HOST: Q[nshell*nshell], symmetric, caller's shell order.  Synchronises. */
+int ltjk_get_schwarz(ltjk_ctx* ctx, double* Q_host);
+
+/* Minimax Laplace quadrature (step a3; Eq. 11): nodes t[npts] and weights w[npts] (HOST,
+ * caller-allocated) minimising max_{x in [xmin,xmax]} |1/x - sum_a w_a exp(-x t_a)|.  *maxerr (may be NULL)
+ * receives the achieved maximum error on [xmin,xmax].  Pure host function; 1 <= npts <= 16.
+ * LTJK_ENOCONV if the Remez iteration fails. */
+int ltjk_laplace_quadrature(double xmin, double xmax, int npts, double* t, double* w, double* maxerr);
+
+/* Pseudo-density transform (step a4; Eq. 13, L145 Eq. 15):
+ *   D_out[a][d][mu][nu] = sum_{i,b} C_occ[mu][i] e^{+eps_occ[i] tau[a]} T[d][i][b] e^{-eps_vir[b] tau[a]} C_vir[nu][b]
+ * DEVICE pointers, row-major, contiguous: C_occ[N][nocc], C_vir[N][nvir], eps_occ[nocc], eps_vir[nvir],
+ * T[nT][nocc][nvir], D_out[ntau][nT][N][N].  tau_host[ntau] is a HOST pointer.  No w_alpha is applied. */
+int ltjk_build_pseudo_densities(ltjk_ctx* ctx, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                                const double* eps_occ, const double* eps_vir, int nT, const double* T,
+                                int ntau, const double* tau_host, double* D_out);
+
+/* Non-symmetric J/K build (steps a5-a9; Eq. 17):
+ *   J[d][mu][nu] = sum_{kappa rho} (mu nu|kappa rho) D[d][kappa][rho]
+ *   K[d][mu][nu] = sum_{kappa rho} (mu kappa|nu rho) D[d][kappa][rho]
+ * over all quartets surviving the Schwarz test.  D is a general real matrix (D != D^T): K comes out as a
+ * full non-symmetric matrix with K[D^T] = K[D]^T; J is symmetric.  DEVICE pointers [nD][N][N], row-major;
+ * J and K are OVERWRITTEN; either may be NULL (J-only / K-only). */
+int ltjk_jk_build(ltjk_ctx* ctx, int nD, const double* D, double* J, double* K);
+
+/* Same as ltjk_jk_build but with HOST buffers: copies D to the device, builds, copies J and K back and
+ * synchronises.  This is the end-to-end entry bench.py times as "e2e". */
+int ltjk_jk_build_host(ltjk_ctx* ctx, int nD, const double* D_host, double* J_host, double* K_host);
+
+/* Statistics of the last ltjk_jk_build on this context (HOST outputs, any may be NULL):
+ *   n_launches    kernels launched
+ *   eri_quartets  contracted shell quartets evaluated (4-fold unique: A>=B, C>=D, all bra x ket)
+ *   digest_flops  fp64 flops of the digestion contractions (2 * M * K * nD summed over tiles)
+ *   eri_ms, digest_ms  device time of the two kernel families (only if timing was enabled, else -1) */
+int ltjk_get_stats(const ltjk_ctx* ctx, long long* n_launches, long long* eri_quartets, double* digest_flops,
+                   double* eri_ms, double* digest_ms);
+int ltjk_set_timing(ltjk_ctx* ctx, int enable);
+
+/* Test hook: contracted Cartesian shell quartet (A B|C D) in the caller's shell indices, evaluated by the
+ * device ERI kernel, written to HOST out[na*nb*nc*nd] (row-major a,b,c,d).  Synchronises. */
+int ltjk_debug_eri_quartet(ltjk_ctx* ctx, int A, int B, int C, int D, double* out_host);
+
+/* Test hook: device Boys function F_m(T), m = 0..mmax (mmax <= 8), for n arguments T_host[n];
+ * F_host[n*(mmax+1)].  Synchronises. */
+int ltjk_debug_boys(ltjk_ctx* ctx, int mmax, int n, const double* T_host, double* F_host);
+
+/* Microbenchmarks that give the roofline denominators: sustained fp64 FMA rate of the
+ * vector pipe (independent DFMA chains on all SMs) in TFLOP/s, and a device copy in GB/s.  Synchronises. */
+int ltjk_bench_dfma_peak(ltjk_ctx* ctx, double* tflops);
+int ltjk_bench_copy_peak(ltjk_ctx* ctx, double* gbs);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LTJK_H */
