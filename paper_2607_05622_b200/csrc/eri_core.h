@@ -98,7 +98,7 @@ LTJK_HD void build_pair_record(const double* A, const double* B, int na, const d
 constexpr double kPrimCut = 1e-20;
 
 // Step a7.  Contracted quartet (ab|cd) -> out[((a*nb+b)*nc+c)*nd+d].
-template <int LA, int LB, int LC, int LD>
+template <int LA, int LB, int LC, int LD, bool CUT = true>
 LTJK_HD void eri_quartet(const double* __restrict__ bra, const double* __restrict__ ket,
                          const double* __restrict__ boys_tab, double* __restrict__ out)
 {
@@ -122,7 +122,7 @@ LTJK_HD void eri_quartet(const double* __restrict__ bra, const double* __restric
             const double q = k[0], Kcd = k[7];
             const double pq = p + q, ipq = 1.0 / pq;
             const double pref = Kab * Kcd * 34.986836655249725693 /* 2 pi^{5/2} */ / (p * q * sqrt(pq));
-            if (fabs(pref) < kPrimCut) continue;
+            if (CUT && fabs(pref) < kPrimCut) continue;   // never for the Schwarz diagonal (Q^2 may be < 1e-20)
             const double PQx = Px - k[1], PQy = Py - k[2], PQz = Pz - k[3];
             const double rho = p * q * ipq;
             const double T = rho * (PQx * PQx + PQy * PQy + PQz * PQz);

@@ -1,0 +1,250 @@
+// ltjk_api.cu -- the C ABI of include/ltjk.h: context, basis upload (a1), shell-pair/Schwarz setup and the
+// geometry-frozen work lists (a2, a5), and the J/K build driver (a5-a9).
+#include "ltjk_internal.h"
+#include "eri_core.h"
+#include "boys_table.h"
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+
+namespace ltjk {
+
+int set_err(ltjk_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg;
+    return code;
+}
+
+void digest_colblocks(int nD, int* TN, int* ncolblk);   // ltjk_digest.cu
+
+static const int kBlkShells[3] = {16, 5, 3};   // target shells per block for l = 0,1,2 (16 / 15 / 18 AOs)
+static const int kRunMax = 8;                  // panels accumulated in registers before a flush
+
+template <class T>
+int upload_impl(ltjk_ctx* c, T** dst, const std::vector<T>& src)
+{
+    if (*dst) { cudaFree(*dst); *dst = nullptr; }
+    if (src.empty()) return LTJK_OK;
+    LTJK_CUDA(c, cudaMalloc((void**)dst, sizeof(T) * src.size()));
+    LTJK_CUDA(c, cudaMemcpyAsync(*dst, src.data(), sizeof(T) * src.size(), cudaMemcpyHostToDevice, c->stream));
+    return LTJK_OK;
+}
+
+void free_tables(ltjk_ctx* c)
+{
+    DevTables& t = c->t;
+    void* ptrs[] = {t.pair_rec, t.schwarz, t.sh_ao, t.blk_sh0, t.blk_nsh, t.blk_ao0, t.blk_nao, t.pair_I, t.pair_J,
+                    t.koff, t.rank_of, t.ao_perm, c->d_items, c->d_panel};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    double* boys = t.boys;
+    t = DevTables();
+    t.boys = boys;
+    c->d_items = nullptr; c->d_panel = nullptr; c->panel_cap = 0; c->n_items = 0;
+    c->have_pairs = false;
+}
+
+void free_work(ltjk_ctx* c)
+{
+    void* ptrs[] = {c->Dt, c->Dst, c->Jt, c->Kt, c->hD, c->hJ, c->hK};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    c->Dt = c->Dst = c->Jt = c->Kt = c->hD = c->hJ = c->hK = nullptr;
+    c->work_cap = 0; c->host_cap = 0;
+}
+
+static inline int pair_class(int la, int lb) { return la * (la + 1) / 2 + lb; }
+
+// Build chunks (bra block pair x a range of ket ranks that fits the panel ring) and their digest items.
+void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
+{
+    const int nblk = (int)c->blk_nao.size(), npair = (int)c->pair_I.size();
+    c->chunks.clear();
+    items.clear();
+    auto rowtiles = [](int rows) { return (rows + 63) / 64; };
+    std::vector<std::vector<int>> byL(nblk);
+    for (int rIJ = 0; rIJ < npair; ++rIJ) {
+        const int I = c->pair_I[rIJ], J = c->pair_J[rIJ];
+        const int nI = c->blk_nao[I], nJ = c->blk_nao[J];
+        const long long cap = std::max<long long>(c->panel_cap / ((long long)nI * nJ), 1);
+        int r0 = 0;
+        while (r0 <= rIJ) {
+            int r1 = r0 + 1;
+            while (r1 <= rIJ && c->koff[r1 + 1] - c->koff[r0] <= cap) ++r1;
+            Chunk ch;
+            ch.I = I; ch.J = J; ch.rIJ = rIJ; ch.r0 = r0; ch.r1 = r1; ch.item0 = (long long)items.size();
+            // ---- J views
+            for (int ra = r0; ra < r1; ra += kRunMax) {
+                const int cnt = std::min(kRunMax, r1 - ra);
+                for (int rt = 0; rt < rowtiles(nI * nJ); ++rt)
+                    items.push_back(DigestItem{0, 0, (unsigned short)rt, ra, 0, cnt});
+            }
+            for (int r = r0; r < r1; ++r) {
+                const int nK = c->blk_nao[c->pair_I[r]], nL = c->blk_nao[c->pair_J[r]];
+                for (int rt = 0; rt < rowtiles(nK * nL); ++rt)
+                    items.push_back(DigestItem{1, 0, (unsigned short)rt, r, 0, 1});
+            }
+            ch.nitemsJ = (int)((long long)items.size() - ch.item0);
+            // ---- K views 2,3: runs of consecutive ranks with the same K (L consecutive by construction)
+            for (int ra = r0; ra < r1;) {
+                const int K = c->pair_I[ra];
+                int rb = ra + 1;
+                while (rb < r1 && c->pair_I[rb] == K && c->pair_J[rb] == c->pair_J[rb - 1] + 1 && rb - ra < kRunMax) ++rb;
+                const int nK = c->blk_nao[K];
+                for (int view = 2; view <= 3; ++view) {
+                    const int rows = (view == 2 ? nI : nJ) * nK;
+                    for (int partner = 0; partner < 2; ++partner)
+                        for (int rt = 0; rt < rowtiles(rows); ++rt)
+                            items.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned short)rt, K,
+                                                       c->pair_J[ra], rb - ra});
+                }
+                ra = rb;
+            }
+            // ---- K views 4,5: for each L, runs of consecutive K
+            for (int r = r0; r < r1; ++r) byL[c->pair_J[r]].push_back(c->pair_I[r]);
+            for (int L = 0; L < nblk; ++L) {
+                std::vector<int>& ks = byL[L];
+                if (ks.empty()) continue;
+                std::sort(ks.begin(), ks.end());
+                const int nL = c->blk_nao[L];
+                for (size_t a = 0; a < ks.size();) {
+                    size_t b = a + 1;
+                    while (b < ks.size() && ks[b] == ks[b - 1] + 1 && (int)(b - a) < kRunMax) ++b;
+                    for (int view = 4; view <= 5; ++view) {
+                        const int rows = (view == 4 ? nI : nJ) * nL;
+                        for (int partner = 0; partner < 2; ++partner)
+                            for (int rt = 0; rt < rowtiles(rows); ++rt)
+                                items.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned short)rt, L,
+                                                           ks[a], (int)(b - a)});
+                    }
+                    a = b;
+                }
+                ks.clear();
+            }
+            ch.nitemsK = (int)((long long)items.size() - ch.item0) - ch.nitemsJ;
+            c->chunks.push_back(ch);
+            r0 = r1;
+        }
+    }
+}
+
+}  // namespace ltjk
+
+using namespace ltjk;
+
+extern "C" {
+
+int ltjk_create(ltjk_ctx** out, int device, void* cuda_stream)
+{
+    if (!out) return LTJK_EINVAL;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return LTJK_ECUDA;   // no CPU fallback
+    if (cudaSetDevice(device) != cudaSuccess) return LTJK_ECUDA;
+    ltjk_ctx* c = new (std::nothrow) ltjk_ctx();
+    if (!c) return LTJK_ENOMEM;
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    std::vector<double> tab = make_boys_table(kBoysNT, kBoysNM);
+    if (cudaMalloc(&c->t.boys, sizeof(double) * tab.size()) != cudaSuccess ||
+        cudaMemcpy(c->t.boys, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+        delete c;
+        return LTJK_ECUDA;
+    }
+    *out = c;
+    return LTJK_OK;
+}
+
+int ltjk_destroy(ltjk_ctx* c)
+{
+    if (!c) return LTJK_EINVAL;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    free_tables(c);
+    free_work(c);
+    if (c->t.boys) cudaFree(c->t.boys);
+    delete c;
+    return LTJK_OK;
+}
+
+const char* ltjk_last_error(const ltjk_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int ltjk_set_scratch_bytes(ltjk_ctx* c, long long bytes)
+{
+    if (!c || bytes < 0) return LTJK_EINVAL;
+    c->scratch_bytes = bytes;
+    return LTJK_OK;
+}
+
+int ltjk_set_basis(ltjk_ctx* c, int natom, const double* xyz, int nshell, const int* atom, const int* l,
+                   const int* nprim, const int* prim_off, const double* exps, const double* coef)
+{
+    if (!c) return LTJK_EINVAL;
+    if (natom <= 0 || nshell <= 0 || !xyz || !atom || !l || !nprim || !prim_off || !exps || !coef)
+        return set_err(c, LTJK_EINVAL, "set_basis: null pointer or non-positive size");
+    int ntot = 0;
+    for (int s = 0; s < nshell; ++s) {
+        if (l[s] < 0) return set_err(c, LTJK_EINVAL, "set_basis: negative angular momentum");
+        if (l[s] > 2) return set_err(c, LTJK_ELMAX, "set_basis: angular momentum > 2 (kernels are Cartesian s, p, d)");
+        if (nprim[s] < 1 || nprim[s] > 4) return set_err(c, LTJK_EINVAL, "set_basis: nprim must be 1..4");
+        if (atom[s] < 0 || atom[s] >= natom || prim_off[s] < 0) return set_err(c, LTJK_EINVAL, "set_basis: bad atom/prim_off");
+        ntot = std::max(ntot, prim_off[s] + nprim[s]);
+    }
+    for (int i = 0; i < ntot; ++i)
+        if (!(exps[i] > 0.0)) return set_err(c, LTJK_EINVAL, "set_basis: exponents must be positive");
+    cudaSetDevice(c->device);
+    free_tables(c);
+    c->natom = natom; c->nshell = nshell;
+    c->xyz.assign(xyz, xyz + 3 * natom);
+    c->atom.assign(atom, atom + nshell); c->l.assign(l, l + nshell);
+    c->nprim.assign(nprim, nprim + nshell); c->prim_off.assign(prim_off, prim_off + nshell);
+    c->exps.assign(exps, exps + ntot); c->coef.assign(coef, coef + ntot);
+
+    // caller AO offsets
+    std::vector<int> ao_ext(nshell + 1, 0);
+    for (int s = 0; s < nshell; ++s) ao_ext[s + 1] = ao_ext[s] + ncart(l[s]);
+    c->nao = ao_ext[nshell];
+    // internal shell order: by l, then caller order
+    c->sh_int2ext.resize(nshell);
+    for (int s = 0; s < nshell; ++s) c->sh_int2ext[s] = s;
+    std::stable_sort(c->sh_int2ext.begin(), c->sh_int2ext.end(), [&](int a, int b) { return l[a] < l[b]; });
+    c->sh_ao_int.assign(nshell, 0);
+    c->ao_perm.assign(c->nao, 0);
+    int ao = 0;
+    for (int s = 0; s < nshell; ++s) {
+        const int e = c->sh_int2ext[s];
+        c->sh_ao_int[s] = ao;
+        for (int k = 0; k < ncart(l[e]); ++k) c->ao_perm[ao++] = ao_ext[e] + k;
+    }
+    // l-homogeneous blocks, evenly split
+    c->blk_sh0.clear(); c->blk_nsh.clear(); c->blk_ao0.clear(); c->blk_nao.clear(); c->blk_l.clear();
+    int s0 = 0;
+    for (int ll = 0; ll < 3; ++ll) {
+        int n = 0;
+        while (s0 + n < nshell && l[c->sh_int2ext[s0 + n]] == ll) ++n;
+        c->max_nsh_l[ll] = 0;
+        if (n == 0) continue;
+        const int nb = (n + kBlkShells[ll] - 1) / kBlkShells[ll];
+        int done = 0;
+        for (int b = 0; b < nb; ++b) {
+            const int cnt = (n - done + (nb - b) - 1) / (nb - b);
+            c->blk_sh0.push_back(s0 + done); c->blk_nsh.push_back(cnt);
+            c->blk_ao0.push_back(c->sh_ao_int[s0 + done]); c->blk_nao.push_back(cnt * ncart(ll));
+            c->blk_l.push_back(ll);
+            c->max_nsh_l[ll] = std::max(c->max_nsh_l[ll], cnt);
+            done += cnt;
+        }
+        s0 += n;
+    }
+    c->have_basis = true;
+    return LTJK_OK;
+}
+
+int ltjk_get_nao(const ltjk_ctx* c, int* nao)
+{
+    if (!c || !nao) return LTJK_EINVAL;
+    if (!c->have_basis) return LTJK_ENOBASIS;
+    *nao = c->nao;
+    return LTJK_OK;
+}
+
+}  // extern "C"

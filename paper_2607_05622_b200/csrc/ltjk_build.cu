@@ -1,0 +1,350 @@
+// ltjk_build.cu -- C ABI, second part: shell-pair/Schwarz setup (a2, a5), the J/K build driver (a5-a9),
+// the pseudo-density entry (a4), statistics, test hooks and the peak microbenchmarks.
+#include "ltjk_internal.h"
+#include "eri_core.h"
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+using namespace ltjk;
+
+namespace {
+
+template <class T>
+int upload(ltjk_ctx* c, T** dst, const std::vector<T>& src)
+{
+    if (*dst) { cudaFree(*dst); *dst = nullptr; }
+    if (src.empty()) return LTJK_OK;
+    LTJK_CUDA(c, cudaMalloc((void**)dst, sizeof(T) * src.size()));
+    LTJK_CUDA(c, cudaMemcpyAsync(*dst, src.data(), sizeof(T) * src.size(), cudaMemcpyHostToDevice, c->stream));
+    return LTJK_OK;
+}
+
+inline int pair_class(int la, int lb) { return la * (la + 1) / 2 + lb; }
+
+int ensure_work(ltjk_ctx* c, int nDp)
+{
+    const long long need = (long long)c->nao * c->nao * nDp;
+    if (need <= c->work_cap) return LTJK_OK;
+    double** bufs[] = {&c->Dt, &c->Dst, &c->Jt, &c->Kt};
+    for (double** b : bufs) {
+        if (*b) { cudaFree(*b); *b = nullptr; }
+        c->work_cap = 0;
+        LTJK_CUDA(c, cudaMalloc((void**)b, sizeof(double) * need));
+    }
+    c->work_cap = need;
+    return LTJK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, long long* n_quartets_kept)
+{
+    if (!c) return LTJK_EINVAL;
+    if (!c->have_basis) return set_err(c, LTJK_ENOBASIS, "build_shell_pairs: no basis");
+    if (!(schwarz_tau >= 0.0)) return set_err(c, LTJK_EINVAL, "build_shell_pairs: negative threshold");
+    cudaSetDevice(c->device);
+    free_tables(c);
+    c->tau = schwarz_tau;
+    const int ns = c->nshell;
+    DevTables& t = c->t;
+    t.nshell = ns; t.nao = c->nao; t.nblk = (int)c->blk_nao.size();
+    int maxnp = 1;
+    for (int s = 0; s < ns; ++s) maxnp = std::max(maxnp, c->nprim[s]);
+    t.rec_stride = kPairHeader + maxnp * maxnp * kPrimStride;
+
+    // ---- a1: basis to the device (temporary, caller order) and a2: pair records + Schwarz bounds
+    double *d_xyz = nullptr, *d_exps = nullptr, *d_coef = nullptr;
+    int *d_atom = nullptr, *d_l = nullptr, *d_nprim = nullptr, *d_poff = nullptr, *d_i2e = nullptr;
+    int rc;
+    if ((rc = upload(c, &d_xyz, c->xyz)) || (rc = upload(c, &d_exps, c->exps)) || (rc = upload(c, &d_coef, c->coef)) ||
+        (rc = upload(c, &d_atom, c->atom)) || (rc = upload(c, &d_l, c->l)) || (rc = upload(c, &d_nprim, c->nprim)) ||
+        (rc = upload(c, &d_poff, c->prim_off)) || (rc = upload(c, &d_i2e, c->sh_int2ext)))
+        return rc;
+    LTJK_CUDA(c, cudaMalloc(&t.pair_rec, sizeof(double) * (size_t)ns * ns * t.rec_stride));
+    LTJK_CUDA(c, cudaMalloc(&t.schwarz, sizeof(double) * (size_t)ns * ns));
+    LTJK_CUDA(c, cudaMemsetAsync(t.schwarz, 0, sizeof(double) * (size_t)ns * ns, c->stream));
+    if ((rc = launch_pair_records(c, d_xyz, d_atom, d_l, d_nprim, d_poff, d_exps, d_coef, d_i2e))) return rc;
+    int lrange[4] = {0, 0, 0, ns};
+    for (int s = 0; s < ns; ++s) {
+        const int ll = c->l[c->sh_int2ext[s]];
+        if (ll < 1) lrange[1] = s + 1;
+        if (ll < 2) lrange[2] = s + 1;
+    }
+    if ((rc = launch_schwarz(c, lrange))) return rc;
+    c->Qhost.assign((size_t)ns * ns, 0.0);
+    LTJK_CUDA(c, cudaMemcpyAsync(c->Qhost.data(), t.schwarz, sizeof(double) * (size_t)ns * ns, cudaMemcpyDeviceToHost,
+                                 c->stream));
+    LTJK_CUDA(c, cudaStreamSynchronize(c->stream));
+    cudaFree(d_xyz); cudaFree(d_exps); cudaFree(d_coef); cudaFree(d_atom); cudaFree(d_l); cudaFree(d_nprim);
+    cudaFree(d_poff); cudaFree(d_i2e);
+
+    // ---- a5: screened quartet count (canonical, shell level): #{(p,q): p >= q, Q_p Q_q >= tau}
+    {
+        std::vector<double> q;
+        q.reserve((size_t)ns * (ns + 1) / 2);
+        for (int A = 0; A < ns; ++A)
+            for (int B = 0; B <= A; ++B) q.push_back(c->Qhost[(size_t)A * ns + B]);
+        std::sort(q.begin(), q.end());
+        long long ordered = 0, diag = 0;
+        for (double v : q) {
+            if (v * v >= schwarz_tau) ++diag;
+            // count w in q with v*w >= tau
+            size_t lo = 0, hi = q.size();
+            while (lo < hi) { const size_t mid = (lo + hi) / 2; if (v * q[mid] >= schwarz_tau) hi = mid; else lo = mid + 1; }
+            ordered += (long long)(q.size() - lo);
+        }
+        c->n_quartets_kept = (ordered + diag) / 2;
+    }
+
+    // ---- block pairs ranked class-major, panel offsets
+    const int nblk = t.nblk;
+    c->pair_I.clear(); c->pair_J.clear();
+    c->rank_of.assign((size_t)nblk * nblk, -1);
+    for (int cls = 0; cls < 6; ++cls)
+        for (int I = 0; I < nblk; ++I)
+            for (int J = 0; J <= I; ++J)
+                if (pair_class(c->blk_l[I], c->blk_l[J]) == cls) {
+                    c->rank_of[(size_t)I * nblk + J] = (int)c->pair_I.size();
+                    c->pair_I.push_back(I); c->pair_J.push_back(J);
+                }
+    const int npair = (int)c->pair_I.size();
+    t.npair = npair;
+    c->koff.assign(npair + 1, 0);
+    long long maxpanel = 0;
+    for (int r = 0; r < npair; ++r) {
+        c->koff[r + 1] = c->koff[r] + (long long)c->blk_nao[c->pair_I[r]] * c->blk_nao[c->pair_J[r]];
+        maxpanel = std::max(maxpanel, (long long)c->blk_nao[c->pair_I[r]] * c->blk_nao[c->pair_J[r]]);
+    }
+    maxpanel *= maxpanel;
+
+    // ---- panel staging ring: L2-sized by default, never below one panel
+    size_t freeb = 0, totb = 0;
+    LTJK_CUDA(c, cudaMemGetInfo(&freeb, &totb));
+    long long bytes = c->scratch_bytes > 0 ? c->scratch_bytes : (64ll << 20);
+    bytes = std::min<long long>(bytes, (long long)(0.6 * (double)freeb));
+    long long total = c->koff[npair] * c->koff[npair];      // never need more than everything at once
+    c->panel_cap = std::max<long long>(std::min<long long>(bytes / 8, total), maxpanel);
+    LTJK_CUDA(c, cudaMalloc(&c->d_panel, sizeof(double) * c->panel_cap));
+
+    std::vector<DigestItem> items;
+    build_work(c, items);
+    c->n_items = (long long)items.size();
+    if ((rc = upload(c, &c->d_items, items)) || (rc = upload(c, &t.sh_ao, c->sh_ao_int)) ||
+        (rc = upload(c, &t.blk_sh0, c->blk_sh0)) || (rc = upload(c, &t.blk_nsh, c->blk_nsh)) ||
+        (rc = upload(c, &t.blk_ao0, c->blk_ao0)) || (rc = upload(c, &t.blk_nao, c->blk_nao)) ||
+        (rc = upload(c, &t.pair_I, c->pair_I)) || (rc = upload(c, &t.pair_J, c->pair_J)) ||
+        (rc = upload(c, &t.koff, c->koff)) || (rc = upload(c, &t.rank_of, c->rank_of)) ||
+        (rc = upload(c, &t.ao_perm, c->ao_perm)))
+        return rc;
+    LTJK_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_pairs = true;
+    if (n_pairs) *n_pairs = (long long)ns * (ns + 1) / 2;
+    if (n_quartets_kept) *n_quartets_kept = c->n_quartets_kept;
+    return LTJK_OK;
+}
+
+int ltjk_get_schwarz(ltjk_ctx* c, double* Q_host)
+{
+    if (!c || !Q_host) return LTJK_EINVAL;
+    if (!c->have_pairs) return set_err(c, LTJK_ENOBASIS, "get_schwarz: shell pairs not built");
+    const int ns = c->nshell;
+    for (int A = 0; A < ns; ++A)
+        for (int B = 0; B < ns; ++B)
+            Q_host[(size_t)c->sh_int2ext[A] * ns + c->sh_int2ext[B]] = c->Qhost[(size_t)A * ns + B];
+    return LTJK_OK;
+}
+
+int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
+{
+    if (!c) return LTJK_EINVAL;
+    if (!c->have_pairs) return set_err(c, LTJK_ENOBASIS, "jk_build: shell pairs not built");
+    if (nD <= 0 || !D || (!J && !K)) return set_err(c, LTJK_EINVAL, "jk_build: bad arguments");
+    cudaSetDevice(c->device);
+    int TN, nb;
+    digest_colblocks(nD, &TN, &nb);
+    const int nDp = TN * nb * 32;
+    int rc;
+    if ((rc = ensure_work(c, nDp))) return rc;
+    c->st_launches = 0; c->st_quartets = 0; c->st_digest_flops = 0.0;
+    c->st_eri_ms = c->timing ? 0.0 : -1.0; c->st_digest_ms = c->timing ? 0.0 : -1.0;
+    if ((rc = launch_pack_densities(c, nD, nDp, D))) return rc;
+    const size_t wbytes = sizeof(double) * (size_t)c->nao * c->nao * nDp;
+    if (J) LTJK_CUDA(c, cudaMemsetAsync(c->Jt, 0, wbytes, c->stream));
+    if (K) LTJK_CUDA(c, cudaMemsetAsync(c->Kt, 0, wbytes, c->stream));
+    cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
+    if (c->timing) { cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventCreate(&e2); }
+
+    // class segments of the rank order
+    int cls_start[7];
+    {
+        int r = 0;
+        for (int cls = 0; cls < 6; ++cls) {
+            cls_start[cls] = r;
+            while (r < (int)c->pair_I.size() && pair_class(c->blk_l[c->pair_I[r]], c->blk_l[c->pair_J[r]]) == cls) ++r;
+        }
+        cls_start[6] = r;
+    }
+    for (const Chunk& ch : c->chunks) {
+        const int cb = pair_class(c->blk_l[ch.I], c->blk_l[ch.J]);
+        if (c->timing) cudaEventRecord(e0, c->stream);
+        for (int ck = 0; ck <= cb; ++ck) {
+            const int ra = std::max(ch.r0, cls_start[ck]), rb = std::min(ch.r1, cls_start[ck + 1]);
+            if (ra >= rb) continue;
+            if ((rc = launch_eri_panels(c, ch, ra, rb, cb, ck))) return rc;
+        }
+        if (c->timing) cudaEventRecord(e1, c->stream);
+        if ((rc = launch_digest(c, ch, nDp, J != nullptr, K != nullptr))) return rc;
+        if (c->timing) {
+            cudaEventRecord(e2, c->stream);
+            cudaEventSynchronize(e2);
+            float a = 0.f, b = 0.f;
+            cudaEventElapsedTime(&a, e0, e1); cudaEventElapsedTime(&b, e1, e2);
+            c->st_eri_ms += a; c->st_digest_ms += b;
+        }
+        // statistics: shell quartets evaluated and digestion flops of this chunk
+        const long long nshI = c->blk_nsh[ch.I], nshJ = c->blk_nsh[ch.J];
+        const long long nIJ = (long long)c->blk_nao[ch.I] * c->blk_nao[ch.J];
+        for (int r = ch.r0; r < ch.r1; ++r)
+            c->st_quartets += nshI * nshJ * c->blk_nsh[c->pair_I[r]] * c->blk_nsh[c->pair_J[r]];
+        const double ints = (double)nIJ * (double)(c->koff[ch.r1] - c->koff[ch.r0]);
+        c->st_digest_flops += 2.0 * ints * nDp * ((J ? 2.0 : 0.0) + (K ? 8.0 : 0.0));
+    }
+    if (c->timing) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2); }
+    if ((rc = launch_unpack_results(c, nD, nDp, J, K))) return rc;
+    return LTJK_OK;
+}
+
+int ltjk_jk_build_host(ltjk_ctx* c, int nD, const double* D_host, double* J_host, double* K_host)
+{
+    if (!c) return LTJK_EINVAL;
+    if (!c->have_pairs) return set_err(c, LTJK_ENOBASIS, "jk_build_host: shell pairs not built");
+    if (nD <= 0 || !D_host || (!J_host && !K_host)) return set_err(c, LTJK_EINVAL, "jk_build_host: bad arguments");
+    cudaSetDevice(c->device);
+    const long long need = (long long)nD * c->nao * c->nao;
+    if (need > c->host_cap) {
+        double** bufs[] = {&c->hD, &c->hJ, &c->hK};
+        for (double** b : bufs) {
+            if (*b) { cudaFree(*b); *b = nullptr; }
+            c->host_cap = 0;
+            LTJK_CUDA(c, cudaMalloc((void**)b, sizeof(double) * need));
+        }
+        c->host_cap = need;
+    }
+    LTJK_CUDA(c, cudaMemcpyAsync(c->hD, D_host, sizeof(double) * need, cudaMemcpyHostToDevice, c->stream));
+    const int rc = ltjk_jk_build(c, nD, c->hD, J_host ? c->hJ : nullptr, K_host ? c->hK : nullptr);
+    if (rc) return rc;
+    if (J_host) LTJK_CUDA(c, cudaMemcpyAsync(J_host, c->hJ, sizeof(double) * need, cudaMemcpyDeviceToHost, c->stream));
+    if (K_host) LTJK_CUDA(c, cudaMemcpyAsync(K_host, c->hK, sizeof(double) * need, cudaMemcpyDeviceToHost, c->stream));
+    LTJK_CUDA(c, cudaStreamSynchronize(c->stream));
+    return LTJK_OK;
+}
+
+int ltjk_build_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                                const double* eps_occ, const double* eps_vir, int nT, const double* T, int ntau,
+                                const double* tau_host, double* D_out)
+{
+    if (!c) return LTJK_EINVAL;
+    if (!c->have_basis) return set_err(c, LTJK_ENOBASIS, "build_pseudo_densities: no basis");
+    if (nocc <= 0 || nvir <= 0 || nT <= 0 || ntau <= 0 || !C_occ || !C_vir || !eps_occ || !eps_vir || !T || !tau_host ||
+        !D_out)
+        return set_err(c, LTJK_EINVAL, "build_pseudo_densities: bad arguments");
+    cudaSetDevice(c->device);
+    return launch_pseudo_densities(c, nocc, nvir, C_occ, C_vir, eps_occ, eps_vir, nT, T, ntau, tau_host, D_out);
+}
+
+int ltjk_get_stats(const ltjk_ctx* c, long long* n_launches, long long* eri_quartets, double* digest_flops,
+                   double* eri_ms, double* digest_ms)
+{
+    if (!c) return LTJK_EINVAL;
+    if (n_launches) *n_launches = c->st_launches;
+    if (eri_quartets) *eri_quartets = c->st_quartets;
+    if (digest_flops) *digest_flops = c->st_digest_flops;
+    if (eri_ms) *eri_ms = c->st_eri_ms;
+    if (digest_ms) *digest_ms = c->st_digest_ms;
+    return LTJK_OK;
+}
+
+int ltjk_set_timing(ltjk_ctx* c, int enable)
+{
+    if (!c) return LTJK_EINVAL;
+    c->timing = enable != 0;
+    return LTJK_OK;
+}
+
+int ltjk_debug_eri_quartet(ltjk_ctx* c, int A, int B, int C, int D, double* out_host)
+{
+    if (!c || !out_host) return LTJK_EINVAL;
+    if (!c->have_pairs) return set_err(c, LTJK_ENOBASIS, "debug_eri_quartet: shell pairs not built");
+    const int ns = c->nshell;
+    if (A < 0 || B < 0 || C < 0 || D < 0 || A >= ns || B >= ns || C >= ns || D >= ns)
+        return set_err(c, LTJK_EINVAL, "debug_eri_quartet: shell index out of range");
+    cudaSetDevice(c->device);
+    // caller -> internal shells, then canonical order (l_a >= l_b, l_c >= l_d, class(ab) >= class(cd))
+    std::vector<int> e2i(ns);
+    for (int s = 0; s < ns; ++s) e2i[c->sh_int2ext[s]] = s;
+    int sh[4] = {A, B, C, D}, pos[4] = {0, 1, 2, 3};   // pos[k] = caller position of canonical slot k
+    auto L = [&](int k) { return c->l[sh[pos[k]]]; };
+    if (L(0) < L(1)) std::swap(pos[0], pos[1]);
+    if (L(2) < L(3)) std::swap(pos[2], pos[3]);
+    if (pair_class(L(0), L(1)) < pair_class(L(2), L(3))) { std::swap(pos[0], pos[2]); std::swap(pos[1], pos[3]); }
+    int n[4], nc[4];
+    for (int k = 0; k < 4; ++k) { nc[k] = ncart(L(k)); n[k] = ncart(c->l[sh[k]]); }
+    const int ntot = n[0] * n[1] * n[2] * n[3];
+    double* d_out = nullptr;
+    LTJK_CUDA(c, cudaMalloc(&d_out, sizeof(double) * ntot));
+    const int rc = launch_eri_single(c, e2i[sh[pos[0]]], e2i[sh[pos[1]]], e2i[sh[pos[2]]], e2i[sh[pos[3]]], L(0), L(1),
+                                     L(2), L(3), d_out);
+    if (rc) { cudaFree(d_out); return rc; }
+    std::vector<double> tmp(ntot);
+    LTJK_CUDA(c, cudaMemcpyAsync(tmp.data(), d_out, sizeof(double) * ntot, cudaMemcpyDeviceToHost, c->stream));
+    LTJK_CUDA(c, cudaStreamSynchronize(c->stream));
+    cudaFree(d_out);
+    // tmp is indexed by canonical slots; scatter back to caller order
+    int idx[4];
+    for (idx[0] = 0; idx[0] < nc[0]; ++idx[0])
+        for (idx[1] = 0; idx[1] < nc[1]; ++idx[1])
+            for (idx[2] = 0; idx[2] < nc[2]; ++idx[2])
+                for (idx[3] = 0; idx[3] < nc[3]; ++idx[3]) {
+                    int ci[4];
+                    for (int k = 0; k < 4; ++k) ci[pos[k]] = idx[k];
+                    out_host[((ci[0] * n[1] + ci[1]) * n[2] + ci[2]) * n[3] + ci[3]] =
+                        tmp[((idx[0] * nc[1] + idx[1]) * nc[2] + idx[2]) * nc[3] + idx[3]];
+                }
+    return LTJK_OK;
+}
+
+int ltjk_debug_boys(ltjk_ctx* c, int mmax, int n, const double* T_host, double* F_host)
+{
+    if (!c || !T_host || !F_host || n <= 0 || mmax < 0 || mmax > 8) return LTJK_EINVAL;
+    cudaSetDevice(c->device);
+    double *dT = nullptr, *dF = nullptr;
+    LTJK_CUDA(c, cudaMalloc(&dT, sizeof(double) * n));
+    LTJK_CUDA(c, cudaMalloc(&dF, sizeof(double) * (size_t)n * (mmax + 1)));
+    LTJK_CUDA(c, cudaMemcpyAsync(dT, T_host, sizeof(double) * n, cudaMemcpyHostToDevice, c->stream));
+    const int rc = launch_boys_debug(c, mmax, n, dT, dF);
+    if (!rc) {
+        LTJK_CUDA(c, cudaMemcpyAsync(F_host, dF, sizeof(double) * (size_t)n * (mmax + 1), cudaMemcpyDeviceToHost, c->stream));
+        LTJK_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    cudaFree(dT); cudaFree(dF);
+    return rc;
+}
+
+int ltjk_bench_dfma_peak(ltjk_ctx* c, double* tflops)
+{
+    if (!c || !tflops) return LTJK_EINVAL;
+    cudaSetDevice(c->device);
+    return bench_dfma(c, tflops);
+}
+
+int ltjk_bench_copy_peak(ltjk_ctx* c, double* gbs)
+{
+    if (!c || !gbs) return LTJK_EINVAL;
+    cudaSetDevice(c->device);
+    return bench_copy(c, gbs);
+}
+
+}  // extern "C"

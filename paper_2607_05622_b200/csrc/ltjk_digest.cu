@@ -1,0 +1,417 @@
+// ltjk_digest.cu -- step a8 (non-symmetric J/K digestion), a9 (finalise) and the layout transforms around them.
+//
+// Digestion as blocked fp64 contractions (no per-integral global atomics; Eq. 25, which the
+// paper realises by one atomicAdd per update).  With densities stored density-fastest, Dt[kappa][rho][d], every one
+// of the ten updates of Eq. 25 / oracle step O6 on a block quartet panel P[i][j][k][l] is a small GEMM
+//     X[(r1,r2), d] += sum_{(c1,c2)} P[r1,r2,c1,c2] * B[(c1,c2), d]
+// with (r1,r2) and (c1,c2) two of the four panel indices:
+//     view 0  JIJ: rows (i,j) cols (k,l)  B = Ds[(k,l)]            -> X_J[(i,j)]     Ds = D + D^T
+//     view 1  JKL: rows (k,l) cols (i,j)  B = Ds[(i,j)]            -> X_J[(k,l)]     J  = X_J + X_J^T
+//     view 2  KIK: rows (i,k) cols (j,l)  B = D[(j,l)] -> K[(i,k)] ; partner B = D[(l,j)] -> K[(k,i)]
+//     view 3  KJK: rows (j,k) cols (i,l)  B = D[(i,l)] -> K[(j,k)] ; partner B = D[(l,i)] -> K[(k,j)]
+//     view 4  KIL: rows (i,l) cols (j,k)  B = D[(j,k)] -> K[(i,l)] ; partner B = D[(k,j)] -> K[(l,i)]
+//     view 5  KJL: rows (j,l) cols (i,k)  B = D[(i,k)] -> K[(j,l)] ; partner B = D[(k,i)] -> K[(l,j)]
+// (the 2 J and 8 K images of a canonical quartet; for D != D^T all eight K images are distinct).
+// One CTA owns a 64-row tile of one output block for all (<= 192) densities, keeps it in registers over a RUN of
+// panels sharing that output block, and flushes once with coalesced fp64 reductions.
+#include "ltjk_internal.h"
+#include <cstdio>
+
+namespace ltjk {
+
+constexpr int kMT = 64;        // rows per CTA
+constexpr int kMTP = 66;       // padded row stride of the A tile in shared memory
+constexpr int kKC = 16;        // contraction chunk
+constexpr int kStages = 3;
+constexpr int kMaxNC = 1024;   // max columns of one panel view (block AO count squared)
+
+struct DigestArgs {
+    DevTables t;
+    const DigestItem* items;
+    const double* panel;
+    const double* Dt;
+    const double* Dst;
+    double* Jt;
+    double* Kt;
+    int I, J, r0;
+    int nDp;
+};
+
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem, bool valid)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    const int sz = valid ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool valid)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    const int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+template <int TN>
+struct DigestSmem {
+    double A[kStages][kKC][kMTP];
+    double B[kStages][kKC][32 * TN];
+    int rowoff[kMT];
+    int acol[kMaxNC];
+    unsigned bcol[kMaxNC];
+};
+
+template <int TN>
+__global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    DigestSmem<TN>& S = *reinterpret_cast<DigestSmem<TN>*>(smem_raw);
+    const DevTables& T = g.t;
+    const DigestItem it = g.items[blockIdx.x];
+    const int n0 = blockIdx.y * (32 * TN);
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int N = T.nao, nDp = g.nDp;
+    const int view = it.view;
+    const bool partner = it.partner != 0;
+    const int I = g.I, J = g.J;
+    const int nI = T.blk_nao[I], nJ = T.blk_nao[J];
+
+    double acc[8][TN];
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int t = 0; t < TN; ++t) acc[r][t] = 0.0;
+
+    int R1 = 0, R2 = 0;                       // row blocks of the LAST step (constant over the run by construction)
+    const double* __restrict__ Bmat = (view <= 1) ? g.Dst : g.Dt;
+    const bool rowContig = (view == 1 || view >= 4);   // l (unit stride) is a row index
+
+    for (int s = 0; s < it.count; ++s) {
+        int K, L, rank;
+        if (view <= 1) { rank = it.a + s; K = T.pair_I[rank]; L = T.pair_J[rank]; }
+        else if (view <= 3) { K = it.a; L = it.b + s; rank = T.rank_of[K * T.nblk + L]; }
+        else { L = it.a; K = it.b + s; rank = T.rank_of[K * T.nblk + L]; }
+        const int nK = T.blk_nao[K], nL = T.blk_nao[L];
+        const double* __restrict__ P = g.panel + (T.koff[rank] - T.koff[g.r0]) * (long long)(nI * nJ);
+        const int sI = nJ * nK * nL, sJ = nK * nL, sK = nL, sL = 1;
+        int C1, C2, sR1, sR2, sC1, sC2;
+        switch (view) {
+        case 0: R1 = I; R2 = J; C1 = K; C2 = L; sR1 = sI; sR2 = sJ; sC1 = sK; sC2 = sL; break;
+        case 1: R1 = K; R2 = L; C1 = I; C2 = J; sR1 = sK; sR2 = sL; sC1 = sI; sC2 = sJ; break;
+        case 2: R1 = I; R2 = K; C1 = J; C2 = L; sR1 = sI; sR2 = sK; sC1 = sJ; sC2 = sL; break;
+        case 3: R1 = J; R2 = K; C1 = I; C2 = L; sR1 = sJ; sR2 = sK; sC1 = sI; sC2 = sL; break;
+        case 4: R1 = I; R2 = L; C1 = J; C2 = K; sR1 = sI; sR2 = sL; sC1 = sJ; sC2 = sK; break;
+        default: R1 = J; R2 = L; C1 = I; C2 = K; sR1 = sJ; sR2 = sL; sC1 = sI; sC2 = sK; break;
+        }
+        const int nR2 = T.blk_nao[R2], nrows = T.blk_nao[R1] * nR2;
+        const int nC2 = T.blk_nao[C2], nC = T.blk_nao[C1] * nC2;
+        const int aoC1 = T.blk_ao0[C1], aoC2 = T.blk_ao0[C2];
+
+        __syncthreads();   // previous step done with tables and stage buffers
+        if (tid < kMT) {
+            const int m = it.rowtile * kMT + tid;
+            S.rowoff[tid] = (m < nrows) ? (m / nR2) * sR1 + (m % nR2) * sR2 : -1;
+        }
+        for (int cidx = tid; cidx < nC; cidx += 256) {
+            const int c1 = cidx / nC2, c2 = cidx % nC2;
+            S.acol[cidx] = c1 * sC1 + c2 * sC2;
+            S.bcol[cidx] = partner ? (unsigned)((aoC2 + c2) * N + aoC1 + c1) : (unsigned)((aoC1 + c1) * N + aoC2 + c2);
+        }
+        __syncthreads();
+
+        const int nch = (nC + kKC - 1) / kKC;
+        auto load = [&](int st, int ch) {
+            // A tile: kKC x kMT elements, 4 per thread
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                int m, k;
+                if (rowContig) { m = tid & 63; k = (tid >> 6) + 4 * e; }
+                else { k = tid & 15; m = (tid >> 4) + 16 * e; }
+                const int cidx = ch * kKC + k;
+                const int ro = S.rowoff[m];
+                const bool ok = (ro >= 0) && (cidx < nC);
+                const double* src = ok ? (P + ro + S.acol[cidx]) : P;
+                cp_async8(&S.A[st][k][m], src, ok);
+            }
+            // B tile: kKC rows of 32*TN doubles, 16-byte pieces
+#pragma unroll
+            for (int e = 0; e < TN; ++e) {
+                const int id = tid + 256 * e;
+                const int k = id / (16 * TN), piece = id % (16 * TN);
+                const int cidx = ch * kKC + k;
+                const bool ok = cidx < nC;
+                const double* src = ok ? (Bmat + (size_t)S.bcol[cidx] * nDp + n0 + piece * 2) : Bmat;
+                cp_async16(&S.B[st][k][piece * 2], src, ok);
+            }
+        };
+#pragma unroll
+        for (int st = 0; st < kStages - 1; ++st) {
+            if (st < nch) load(st, st);
+            cp_async_commit();
+        }
+        for (int ch = 0; ch < nch; ++ch) {
+            cp_async_wait<kStages - 2>();
+            __syncthreads();
+            const int nxt = ch + kStages - 1;
+            if (nxt < nch) load(nxt % kStages, nxt);
+            cp_async_commit();
+            const int st = ch % kStages;
+#pragma unroll
+            for (int k = 0; k < kKC; ++k) {
+                const double2* ap = reinterpret_cast<const double2*>(&S.A[st][k][w * 8]);
+                const double2 a01 = ap[0], a23 = ap[1], a45 = ap[2], a67 = ap[3];
+                const double a[8] = {a01.x, a01.y, a23.x, a23.y, a45.x, a45.y, a67.x, a67.y};
+                double b[TN];
+#pragma unroll
+                for (int t = 0; t < TN; ++t) b[t] = S.B[st][k][lane + 32 * t];
+#pragma unroll
+                for (int r = 0; r < 8; ++r)
+#pragma unroll
+                    for (int t = 0; t < TN; ++t) acc[r][t] = fma(a[r], b[t], acc[r][t]);
+            }
+        }
+        cp_async_wait<0>();
+    }
+
+    // flush: coalesced fp64 reductions into the density-fastest accumulators
+    double* __restrict__ Out = (view <= 1) ? g.Jt : g.Kt;
+    const int nR2 = T.blk_nao[R2], nrows = T.blk_nao[R1] * nR2;
+    const int aoR1 = T.blk_ao0[R1], aoR2 = T.blk_ao0[R2];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int m = it.rowtile * kMT + w * 8 + r;
+        if (m < nrows) {
+            const int r1 = m / nR2, r2 = m % nR2;
+            const size_t row = partner ? (size_t)(aoR2 + r2) * N + aoR1 + r1 : (size_t)(aoR1 + r1) * N + aoR2 + r2;
+            double* o = Out + row * nDp + n0 + lane;
+#pragma unroll
+            for (int t = 0; t < TN; ++t) atomicAdd(o + 32 * t, acc[r][t]);
+        }
+    }
+}
+
+template <int TN>
+static int launch_digest_tn(ltjk_ctx* c, const DigestArgs& g, int nitems, int ncolblk)
+{
+    const size_t smem = sizeof(DigestSmem<TN>);
+    static bool attr_set = false;
+    if (!attr_set) {
+        LTJK_CUDA(c, cudaFuncSetAttribute(digest_kernel<TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    digest_kernel<TN><<<dim3(nitems, ncolblk), 256, smem, c->stream>>>(g);
+    LTJK_CUDA(c, cudaGetLastError());
+    return LTJK_OK;
+}
+
+// column blocking of the padded density count: nDp = ncolblk * 32 * TN
+void digest_colblocks(int nD, int* TN, int* ncolblk)
+{   // declared in ltjk_internal.h
+    const int n32 = (nD + 31) / 32;
+    int best_tn = 1, best_nb = n32, best_cost = 1 << 30;
+    for (int tn = 1; tn <= 6; ++tn) {
+        const int nb = (n32 + tn - 1) / tn;
+        const int cost = nb * tn * 8 + nb * 3;   // padded columns, then fewer passes over A
+        if (cost < best_cost) { best_cost = cost; best_tn = tn; best_nb = nb; }
+    }
+    *TN = best_tn; *ncolblk = best_nb;
+}
+
+int launch_digest(ltjk_ctx* c, const Chunk& ch, int nDp, bool doJ, bool doK)
+{
+    const long long first = ch.item0 + (doJ ? 0 : ch.nitemsJ);
+    const int nitems = (doJ ? ch.nitemsJ : 0) + (doK ? ch.nitemsK : 0);
+    if (nitems == 0) return LTJK_OK;
+    DigestArgs g;
+    g.t = c->t; g.items = c->d_items + first; g.panel = c->d_panel;
+    g.Dt = c->Dt; g.Dst = c->Dst; g.Jt = c->Jt; g.Kt = c->Kt;
+    g.I = ch.I; g.J = ch.J; g.r0 = ch.r0; g.nDp = nDp;
+    int TN, nb;
+    digest_colblocks(nDp, &TN, &nb);
+    if (nb * TN * 32 != nDp) return set_err(c, LTJK_EINVAL, "internal: nDp is not a whole number of column blocks");
+    c->st_launches++;
+    switch (TN) {
+    case 1: return launch_digest_tn<1>(c, g, nitems, nb);
+    case 2: return launch_digest_tn<2>(c, g, nitems, nb);
+    case 3: return launch_digest_tn<3>(c, g, nitems, nb);
+    case 4: return launch_digest_tn<4>(c, g, nitems, nb);
+    case 5: return launch_digest_tn<5>(c, g, nitems, nb);
+    default: return launch_digest_tn<6>(c, g, nitems, nb);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Layout transforms (HBM-bound): caller layout X[d][mu][nu] <-> internal density-fastest Xt[mu'][nu'][d'],
+// mu' = internal AO (ao_perm[mu'] = caller AO), d' < nDp (zero padded).
+__global__ void pack_kernel(int N, int nD, int nDp, const int* __restrict__ perm, const double* __restrict__ D,
+                            double* __restrict__ Dt)
+{
+    __shared__ double tile[32][33];
+    const int mu = blockIdx.z, nu0 = blockIdx.x * 32, d0 = blockIdx.y * 32;
+    const int pm = perm[mu];
+    {
+        const int nu = nu0 + threadIdx.x;
+        for (int dd = threadIdx.y; dd < 32; dd += 8) {
+            const int d = d0 + dd;
+            tile[dd][threadIdx.x] = (nu < N && d < nD) ? D[((size_t)d * N + pm) * N + perm[nu]] : 0.0;
+        }
+    }
+    __syncthreads();
+    {
+        const int d = d0 + threadIdx.x;
+        for (int nn = threadIdx.y; nn < 32; nn += 8) {
+            const int nu = nu0 + nn;
+            if (nu < N && d < nDp) Dt[((size_t)mu * N + nu) * nDp + d] = tile[threadIdx.x][nn];
+        }
+    }
+}
+
+__global__ void symmetrize_kernel(int N, int nDp, const double* __restrict__ Dt, double* __restrict__ Dst)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t tot = (size_t)N * N * nDp;
+    if (i >= tot) return;
+    const int d = (int)(i % nDp);
+    const size_t mn = i / nDp;
+    const int mu = (int)(mn / N), nu = (int)(mn % N);
+    Dst[i] = Dt[i] + Dt[((size_t)nu * N + mu) * nDp + d];
+}
+
+// a9: K[d][mu][nu] = Kt[mu'][nu'][d];  J[d][mu][nu] = Xt[mu'][nu'][d] + Xt[nu'][mu'][d]
+__global__ void unpack_kernel(int N, int nD, int nDp, const int* __restrict__ perm, const double* __restrict__ Xt,
+                              double* __restrict__ X, int mirror)
+{
+    __shared__ double tile[32][33];
+    const int mu = blockIdx.z, nu0 = blockIdx.x * 32, d0 = blockIdx.y * 32;
+    {
+        const int d = d0 + threadIdx.x;
+        for (int nn = threadIdx.y; nn < 32; nn += 8) {
+            const int nu = nu0 + nn;
+            double v = 0.0;
+            if (nu < N && d < nDp) {
+                v = Xt[((size_t)mu * N + nu) * nDp + d];
+                if (mirror) v += Xt[((size_t)nu * N + mu) * nDp + d];
+            }
+            tile[nn][threadIdx.x] = v;
+        }
+    }
+    __syncthreads();
+    {
+        const int pm = perm[mu];
+        const int nu = nu0 + threadIdx.x;
+        for (int dd = threadIdx.y; dd < 32; dd += 8) {
+            const int d = d0 + dd;
+            if (nu < N && d < nD) X[((size_t)d * N + pm) * N + perm[nu]] = tile[threadIdx.x][dd];
+        }
+    }
+}
+
+int launch_pack_densities(ltjk_ctx* c, int nD, int nDp, const double* D)
+{
+    const int N = c->nao;
+    dim3 grid((N + 31) / 32, nDp / 32, N), blk(32, 8);
+    pack_kernel<<<grid, blk, 0, c->stream>>>(N, nD, nDp, c->t.ao_perm, D, c->Dt);
+    LTJK_CUDA(c, cudaGetLastError());
+    const size_t tot = (size_t)N * N * nDp;
+    symmetrize_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, c->stream>>>(N, nDp, c->Dt, c->Dst);
+    LTJK_CUDA(c, cudaGetLastError());
+    c->st_launches += 2;
+    return LTJK_OK;
+}
+
+int launch_unpack_results(ltjk_ctx* c, int nD, int nDp, double* J, double* K)
+{
+    const int N = c->nao;
+    dim3 grid((N + 31) / 32, nDp / 32, N), blk(32, 8);
+    if (J) {
+        unpack_kernel<<<grid, blk, 0, c->stream>>>(N, nD, nDp, c->t.ao_perm, c->Jt, J, 1);
+        LTJK_CUDA(c, cudaGetLastError());
+        c->st_launches++;
+    }
+    if (K) {
+        unpack_kernel<<<grid, blk, 0, c->stream>>>(N, nD, nDp, c->t.ao_perm, c->Kt, K, 0);
+        LTJK_CUDA(c, cudaGetLastError());
+        c->st_launches++;
+    }
+    return LTJK_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Roofline denominators: sustained DFMA rate of the fp64 vector pipe, and a device copy.
+__global__ void __launch_bounds__(256) dfma_kernel(int iters, double seed, double* out)
+{
+    double x[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = seed + threadIdx.x * 1e-9 + i;
+    const double a = 1.0000000001, b = 1e-12;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = fma(x[i], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += x[i];
+    if (s == 123.456) out[0] = s;
+}
+
+int bench_dfma(ltjk_ctx* c, double* tflops)
+{
+    cudaDeviceProp prop;
+    LTJK_CUDA(c, cudaGetDeviceProperties(&prop, c->device));
+    double* d = nullptr;
+    LTJK_CUDA(c, cudaMalloc(&d, 8));
+    const int blocks = prop.multiProcessorCount * 8, iters = 1 << 15;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    dfma_kernel<<<blocks, 256, 0, c->stream>>>(1 << 10, 1.0, d);   // warm-up
+    double best = 0.0;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(e0, c->stream);
+        for (int k = 0; k < 8; ++k) dfma_kernel<<<blocks, 256, 0, c->stream>>>(iters, 1.0, d);   // ~0.3 s sustained
+        cudaEventRecord(e1, c->stream);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double fl = 8.0 * blocks * 256.0 * iters * 16.0 * 2.0;
+        best = fmax(best, fl / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(d);
+    LTJK_CUDA(c, cudaGetLastError());
+    *tflops = best;
+    return LTJK_OK;
+}
+
+__global__ void copy_kernel(size_t n, const double2* __restrict__ a, double2* __restrict__ b)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) b[i] = a[i];
+}
+
+int bench_copy(ltjk_ctx* c, double* gbs)
+{
+    const size_t bytes = (size_t)1 << 30;
+    double2 *a = nullptr, *b = nullptr;
+    LTJK_CUDA(c, cudaMalloc(&a, bytes));
+    LTJK_CUDA(c, cudaMalloc(&b, bytes));
+    cudaMemsetAsync(a, 0, bytes, c->stream);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(e0, c->stream);
+        copy_kernel<<<148 * 16, 512, 0, c->stream>>>(bytes / 16, a, b);
+        cudaEventRecord(e1, c->stream);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0) best = fmax(best, 2.0 * bytes / (ms * 1e-3) / 1e9);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(a); cudaFree(b);
+    LTJK_CUDA(c, cudaGetLastError());
+    *gbs = best;
+    return LTJK_OK;
+}
+
+}  // namespace ltjk

@@ -1,0 +1,264 @@
+// ltjk_eri.cu -- steps a2 (shell-pair records, Schwarz bounds), a6+a7 (Boys + OS/HGP shell quartets) as kernels.
+//
+// Integral panels.  A canonical block quartet (IJ|KL) (blocks = l-homogeneous groups of ~16 AOs, see
+// ltjk_internal.h) owns a dense panel  P[i][j][k][l] = s * (ij|kl),  i in I, j in J, k in K, l in L,
+// s = 1/2 per coincidence I==J, K==L, (IJ)==(KL)  (the "canonical-fold multiplicity" of PAPER.md:L320-322 Eq. 25,
+// DESIGN.md reading A4, applied at block level).  Panels live in an L2-sized staging ring, are written here by one
+// thread per contracted shell quartet (the paper's mapping) and are consumed by the
+// digestion kernels (ltjk_digest.cu) before the ring is reused: integrals never form a stored N^4 object.
+// Shell quartets with Q_AB Q_CD < tau (reading A9) are written as zeros.
+#include "ltjk_internal.h"
+#include "eri_core.h"
+#include "boys_table.h"
+
+namespace ltjk {
+
+// ---------------------------------------------------------------------------------------------------------------
+// a2: one thread per ordered internal shell pair (A,B) with l_A >= l_B: Gaussian-product record.
+__global__ void pair_record_kernel(int nshell, const double* __restrict__ xyz, const int* __restrict__ atom,
+                                   const int* __restrict__ l, const int* __restrict__ nprim,
+                                   const int* __restrict__ poff, const double* __restrict__ exps,
+                                   const double* __restrict__ coef, const int* __restrict__ int2ext,
+                                   int rec_stride, double* __restrict__ rec)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nshell * nshell) return;
+    const int A = t / nshell, B = t % nshell;
+    const int a = int2ext[A], b = int2ext[B];
+    if (l[a] < l[b]) return;
+    build_pair_record(xyz + 3 * atom[a], xyz + 3 * atom[b], nprim[a], exps + poff[a], coef + poff[a], nprim[b],
+                      exps + poff[b], coef + poff[b], rec + (size_t)t * rec_stride);
+}
+
+int launch_pair_records(ltjk_ctx* c, const double* d_xyz, const int* d_atom, const int* d_l, const int* d_nprim,
+                        const int* d_poff, const double* d_exps, const double* d_coef, const int* d_int2ext)
+{
+    const int n = c->nshell * c->nshell;
+    pair_record_kernel<<<(n + 127) / 128, 128, 0, c->stream>>>(c->nshell, d_xyz, d_atom, d_l, d_nprim, d_poff, d_exps,
+                                                              d_coef, d_int2ext, c->t.rec_stride, c->t.pair_rec);
+    LTJK_CUDA(c, cudaGetLastError());
+    return LTJK_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a2: Schwarz bounds Q_AB = sqrt(max_{a,b} |(ab|ab)|), one thread per shell pair of class (LA,LB).
+template <int LA, int LB>
+__global__ void schwarz_kernel(int nshell, int a0, int na, int b0, int nb, const double* __restrict__ rec,
+                               int rec_stride, const double* __restrict__ boys, double* __restrict__ Q)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= na * nb) return;
+    const int A = a0 + t / nb, B = b0 + t % nb;
+    if (LA == LB && B > A) return;
+    constexpr int NA = ncart(LA), NB = ncart(LB);
+    double out[NA * NB * NA * NB];
+    const double* r = rec + ((size_t)A * nshell + B) * rec_stride;
+    eri_quartet<LA, LB, LA, LB, false>(r, r, boys, out);
+    double m = 0.0;
+#pragma unroll
+    for (int i = 0; i < NA * NB; ++i) m = fmax(m, fabs(out[i * NA * NB + i]));
+    m = sqrt(m);
+    Q[(size_t)A * nshell + B] = m;
+    Q[(size_t)B * nshell + A] = m;
+}
+
+int launch_schwarz(ltjk_ctx* c, const int* lrange /* host: first internal shell of l = 0,1,2 and end */)
+{
+    const int ns = c->nshell;
+#define SCHW(LA, LB)                                                                                              \
+    {                                                                                                             \
+        const int a0 = lrange[LA], na = lrange[LA + 1] - lrange[LA], b0 = lrange[LB], nb = lrange[LB + 1] - lrange[LB]; \
+        if (na > 0 && nb > 0) {                                                                                   \
+            schwarz_kernel<LA, LB><<<(na * nb + 63) / 64, 64, 0, c->stream>>>(ns, a0, na, b0, nb, c->t.pair_rec,  \
+                                                                              c->t.rec_stride, c->t.boys, c->t.schwarz); \
+            LTJK_CUDA(c, cudaGetLastError());                                                                     \
+        }                                                                                                         \
+    }
+    SCHW(0, 0) SCHW(1, 0) SCHW(1, 1) SCHW(2, 0) SCHW(2, 1) SCHW(2, 2)
+#undef SCHW
+    return LTJK_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a6 + a7: panels of one class segment.  Thread -> (ket rank r in [ra,rb), shell quartet inside the block quartet).
+struct EriArgs {
+    DevTables t;
+    int I, J, rIJ, r0;     // chunk: bra blocks, bra rank, first ket rank of the chunk (panel base origin)
+    int ra, rb;            // ket ranks of this launch (one pair class)
+    int mJ, mK, mL;        // max shells per block of the launch's l_J, l_K, l_L (thread-index decode)
+    int qn;                // mI*mJ*mK*mL
+    double tau;
+    double* panel;
+};
+
+template <int LA, int LB, int LC, int LD>
+__global__ void __launch_bounds__(64) eri_panel_kernel(const EriArgs g)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = g.ra + (int)(t / g.qn);
+    if (r >= g.rb) return;
+    int q = (int)(t % g.qn);
+    const int sd = q % g.mL; q /= g.mL;
+    const int sc = q % g.mK; q /= g.mK;
+    const int sb = q % g.mJ;
+    const int sa = q / g.mJ;
+    const DevTables& T = g.t;
+    const int I = g.I, J = g.J, K = T.pair_I[r], L = T.pair_J[r];
+    if (sa >= T.blk_nsh[I] || sb >= T.blk_nsh[J] || sc >= T.blk_nsh[K] || sd >= T.blk_nsh[L]) return;
+    const int A = T.blk_sh0[I] + sa, B = T.blk_sh0[J] + sb, C = T.blk_sh0[K] + sc, D = T.blk_sh0[L] + sd;
+    constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
+    const int nJ = T.blk_nao[J], nK = T.blk_nao[K], nL = T.blk_nao[L];
+    const long long base = (T.koff[r] - T.koff[g.r0]) * (long long)(T.blk_nao[I] * nJ);
+    double* __restrict__ P = g.panel + base + ((long long)(sa * NA) * nJ + sb * NB) * (nK * nL) + (sc * NC) * nL + sd * ND;
+    const int sI = nJ * nK * nL, sJ = nK * nL, sK = nL;
+
+    const double qq = T.schwarz[(size_t)A * T.nshell + B] * T.schwarz[(size_t)C * T.nshell + D];
+    if (qq < g.tau) {
+        for (int a = 0; a < NA; ++a)
+            for (int b = 0; b < NB; ++b)
+                for (int cc = 0; cc < NC; ++cc)
+#pragma unroll
+                    for (int d = 0; d < ND; ++d) P[a * sI + b * sJ + cc * sK + d] = 0.0;
+        return;
+    }
+    double scale = 1.0;
+    if (I == J) scale *= 0.5;
+    if (K == L) scale *= 0.5;
+    if (r == g.rIJ) scale *= 0.5;
+    double out[NA * NB * NC * ND];
+    eri_quartet<LA, LB, LC, LD>(T.pair_rec + ((size_t)A * T.nshell + B) * T.rec_stride,
+                                T.pair_rec + ((size_t)C * T.nshell + D) * T.rec_stride, T.boys, out);
+    for (int a = 0; a < NA; ++a)
+        for (int b = 0; b < NB; ++b)
+            for (int cc = 0; cc < NC; ++cc)
+#pragma unroll
+                for (int d = 0; d < ND; ++d)
+                    P[a * sI + b * sJ + cc * sK + d] = scale * out[((a * NB + b) * NC + cc) * ND + d];
+}
+
+static const int kClsLa[6] = {0, 1, 1, 2, 2, 2}, kClsLb[6] = {0, 0, 1, 0, 1, 2};
+
+template <int CB, int CK>
+static int launch_cls(ltjk_ctx* c, const EriArgs& g)
+{
+    constexpr int la[6] = {0, 1, 1, 2, 2, 2}, lb[6] = {0, 0, 1, 0, 1, 2};
+    if constexpr (CK <= CB) {
+        const long long nthr = (long long)(g.rb - g.ra) * g.qn;
+        const int bs = 64;
+        eri_panel_kernel<la[CB], lb[CB], la[CK], lb[CK]><<<(unsigned)((nthr + bs - 1) / bs), bs, 0, c->stream>>>(g);
+        LTJK_CUDA(c, cudaGetLastError());
+        return LTJK_OK;
+    } else {
+        return set_err(c, LTJK_EINVAL, "internal: ket class above bra class");
+    }
+}
+
+template <int CB>
+static int launch_cls_k(ltjk_ctx* c, int ck, const EriArgs& g)
+{
+    switch (ck) {
+    case 0: return launch_cls<CB, 0>(c, g);
+    case 1: return launch_cls<CB, 1>(c, g);
+    case 2: return launch_cls<CB, 2>(c, g);
+    case 3: return launch_cls<CB, 3>(c, g);
+    case 4: return launch_cls<CB, 4>(c, g);
+    default: return launch_cls<CB, 5>(c, g);
+    }
+}
+
+int launch_eri_panels(ltjk_ctx* c, const Chunk& ch, int ra, int rb, int cb, int ck)
+{
+    EriArgs g;
+    g.t = c->t;
+    g.I = ch.I; g.J = ch.J; g.rIJ = ch.rIJ; g.r0 = ch.r0; g.ra = ra; g.rb = rb;
+    const int mI = c->max_nsh_l[kClsLa[cb]];
+    g.mJ = c->max_nsh_l[kClsLb[cb]]; g.mK = c->max_nsh_l[kClsLa[ck]]; g.mL = c->max_nsh_l[kClsLb[ck]];
+    g.qn = mI * g.mJ * g.mK * g.mL;
+    g.tau = c->tau;
+    g.panel = c->d_panel;
+    c->st_launches++;
+    switch (cb) {
+    case 0: return launch_cls_k<0>(c, ck, g);
+    case 1: return launch_cls_k<1>(c, ck, g);
+    case 2: return launch_cls_k<2>(c, ck, g);
+    case 3: return launch_cls_k<3>(c, ck, g);
+    case 4: return launch_cls_k<4>(c, ck, g);
+    default: return launch_cls_k<5>(c, ck, g);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Test hooks.
+template <int LA, int LB, int LC, int LD>
+__global__ void eri_single_kernel(const double* bra, const double* ket, const double* boys, double* out)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        double o[ncart(LA) * ncart(LB) * ncart(LC) * ncart(LD)];
+        eri_quartet<LA, LB, LC, LD>(bra, ket, boys, o);
+        for (int i = 0; i < ncart(LA) * ncart(LB) * ncart(LC) * ncart(LD); ++i) out[i] = o[i];
+    }
+}
+
+template <int CB, int CK>
+static void single_cls(ltjk_ctx* c, const double* bra, const double* ket, double* out)
+{
+    constexpr int la[6] = {0, 1, 1, 2, 2, 2}, lb[6] = {0, 0, 1, 0, 1, 2};
+    if constexpr (CK <= CB)
+        eri_single_kernel<la[CB], lb[CB], la[CK], lb[CK]><<<1, 32, 0, c->stream>>>(bra, ket, c->t.boys, out);
+}
+
+template <int CB>
+static void single_cls_k(ltjk_ctx* c, int ck, const double* bra, const double* ket, double* out)
+{
+    switch (ck) {
+    case 0: single_cls<CB, 0>(c, bra, ket, out); break;
+    case 1: single_cls<CB, 1>(c, bra, ket, out); break;
+    case 2: single_cls<CB, 2>(c, bra, ket, out); break;
+    case 3: single_cls<CB, 3>(c, bra, ket, out); break;
+    case 4: single_cls<CB, 4>(c, bra, ket, out); break;
+    default: single_cls<CB, 5>(c, bra, ket, out); break;
+    }
+}
+
+// (AB|CD) for INTERNAL shell indices with l_A>=l_B, l_C>=l_D and class(AB) >= class(CD); d_out row-major a,b,c,d.
+int launch_eri_single(ltjk_ctx* c, int A, int B, int C, int D, int la, int lb, int lc, int ld, double* d_out)
+{
+    const int cb = la * (la + 1) / 2 + lb, ck = lc * (lc + 1) / 2 + ld;
+    const double* bra = c->t.pair_rec + ((size_t)A * c->nshell + B) * c->t.rec_stride;
+    const double* ket = c->t.pair_rec + ((size_t)C * c->nshell + D) * c->t.rec_stride;
+    switch (cb) {
+    case 0: single_cls_k<0>(c, ck, bra, ket, d_out); break;
+    case 1: single_cls_k<1>(c, ck, bra, ket, d_out); break;
+    case 2: single_cls_k<2>(c, ck, bra, ket, d_out); break;
+    case 3: single_cls_k<3>(c, ck, bra, ket, d_out); break;
+    case 4: single_cls_k<4>(c, ck, bra, ket, d_out); break;
+    default: single_cls_k<5>(c, ck, bra, ket, d_out); break;
+    }
+    LTJK_CUDA(c, cudaGetLastError());
+    return LTJK_OK;
+}
+
+template <int M>
+__global__ void boys_debug_kernel(int n, const double* T, const double* tab, double* F)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double f[M + 1];
+    boys_scaled<M>(T[i], 1.0, tab, f);
+    for (int m = 0; m <= M; ++m) F[(size_t)i * (M + 1) + m] = f[m];
+}
+
+int launch_boys_debug(ltjk_ctx* c, int mmax, int n, const double* d_T, double* d_F)
+{
+    const int g = (n + 127) / 128;
+    switch (mmax) {
+#define BD(M) case M: boys_debug_kernel<M><<<g, 128, 0, c->stream>>>(n, d_T, c->t.boys, d_F); break;
+        BD(0) BD(1) BD(2) BD(3) BD(4) BD(5) BD(6) BD(7) BD(8)
+#undef BD
+    default: return set_err(c, LTJK_EINVAL, "mmax must be 0..8");
+    }
+    LTJK_CUDA(c, cudaGetLastError());
+    return LTJK_OK;
+}
+
+}  // namespace ltjk

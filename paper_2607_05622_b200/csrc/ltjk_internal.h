@@ -1,0 +1,132 @@
+// ltjk_internal.h -- context and device-side tables shared by the translation units of libltjk.so.
+// Not part of the C ABI (include/ltjk.h is).  See DESIGN.md for the data layout.
+#pragma once
+#include <cuda_runtime.h>
+#include <string>
+#include <vector>
+#include "../../include/ltjk.h"
+
+namespace ltjk {
+
+// ---- geometry-frozen device tables (built by ltjk_build_shell_pairs, reused by every jk_build) ----------------
+// Shells are re-ordered internally by angular momentum and cut into l-homogeneous BLOCKS of ~16 AOs; block
+// pairs (I>=J) are ranked class-major ((ss),(ps),(pp),(ds),(dp),(dd)), so that every canonical block quartet
+// (IJ|KL), rank(IJ) >= rank(KL), has bra class >= ket class and every panel is class-homogeneous.
+struct DevTables {
+    int nshell = 0, nao = 0, nblk = 0, npair = 0;
+    int rec_stride = 0;            // doubles per shell-pair record
+    double* pair_rec = nullptr;    // [nshell*nshell] records, internal shell order, valid for lA >= lB
+    double* schwarz = nullptr;     // [nshell*nshell] Q_AB, internal shell order
+    double* boys = nullptr;        // Boys table
+    int* sh_ao = nullptr;          // [nshell]   first internal AO of each internal shell
+    int* blk_sh0 = nullptr;        // [nblk]     first internal shell
+    int* blk_nsh = nullptr;        // [nblk]
+    int* blk_ao0 = nullptr;        // [nblk]     first internal AO
+    int* blk_nao = nullptr;        // [nblk]
+    int* pair_I = nullptr;         // [npair]    block pair of rank r
+    int* pair_J = nullptr;
+    long long* koff = nullptr;     // [npair+1]  prefix sum of nao(I)*nao(J) over ranks
+    int* rank_of = nullptr;        // [nblk*nblk] rank of block pair (I,J), I>=J (else -1)
+    int* ao_perm = nullptr;        // [nao]      internal AO -> caller AO
+};
+
+// One digestion work item (16 bytes): a row tile of one output block accumulated over a run of panels.
+struct DigestItem {
+    unsigned char view;     // 0 JIJ, 1 JKL, 2 KIK, 3 KJK, 4 KIL, 5 KJL
+    unsigned char partner;  // K views: 0 -> K[(r1,r2)] with D[(c1,c2)];  1 -> K[(r2,r1)] with D[(c2,c1)]
+    unsigned short rowtile;
+    int a;                  // JIJ/JKL: first ket rank;  KIK/KJK: K;  KIL/KJL: L
+    int b;                  // KIK/KJK: first L;  KIL/KJL: first K
+    int count;              // panels in the run
+};
+
+struct Chunk {
+    int I, J, rIJ;          // bra block pair and its rank
+    int r0, r1;             // ket ranks [r0, r1)
+    long long item0;        // first digest item: nitemsJ J-view items, then nitemsK K-view items
+    int nitemsJ, nitemsK;
+};
+
+}  // namespace ltjk
+
+struct ltjk_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    long long scratch_bytes = 0;   // requested cap (0 = default)
+
+    // basis, caller order (host)
+    int natom = 0, nshell = 0, nao = 0;
+    std::vector<double> xyz, exps, coef;
+    std::vector<int> atom, l, nprim, prim_off;
+    bool have_basis = false, have_pairs = false;
+
+    // internal ordering (host)
+    std::vector<int> sh_int2ext;          // internal shell -> caller shell
+    std::vector<int> sh_ao_int;           // internal shell -> first internal AO
+    std::vector<int> ao_perm;             // internal AO -> caller AO
+    std::vector<int> blk_sh0, blk_nsh, blk_ao0, blk_nao, blk_l;
+    std::vector<int> pair_I, pair_J, rank_of;
+    std::vector<long long> koff;
+    std::vector<double> Qhost;            // internal order [nshell*nshell]
+    std::vector<ltjk::Chunk> chunks;
+    int max_nsh_l[3] = {0, 0, 0};         // max shells per block for each l
+    double tau = 0.0;
+    long long n_quartets_kept = 0;
+
+    ltjk::DevTables t;
+    ltjk::DigestItem* d_items = nullptr;
+    long long n_items = 0;
+    double* d_panel = nullptr;            // integral panel staging ring (L2-sized)
+    long long panel_cap = 0;              // doubles
+
+    // per-build work buffers (grown on demand): density-fastest internal layouts [N][N][nDp]
+    double *Dt = nullptr, *Dst = nullptr, *Jt = nullptr, *Kt = nullptr;
+    long long work_cap = 0;               // doubles per buffer
+    double *hD = nullptr, *hJ = nullptr, *hK = nullptr;   // device staging for jk_build_host
+    long long host_cap = 0;
+
+    // stats
+    long long st_launches = 0, st_quartets = 0;
+    double st_digest_flops = 0.0, st_eri_ms = -1.0, st_digest_ms = -1.0;
+    bool timing = false;
+};
+
+namespace ltjk {
+
+int set_err(ltjk_ctx* c, int code, const std::string& msg);
+#define LTJK_CUDA(c, call)                                                                            \
+    do {                                                                                              \
+        cudaError_t e_ = (call);                                                                      \
+        if (e_ != cudaSuccess)                                                                        \
+            return ltjk::set_err((c), e_ == cudaErrorMemoryAllocation ? LTJK_ENOMEM : LTJK_ECUDA,     \
+                                 std::string(#call) + ": " + cudaGetErrorString(e_));                 \
+    } while (0)
+
+// ltjk_api.cu
+void free_tables(ltjk_ctx* c);
+void free_work(ltjk_ctx* c);
+void build_work(ltjk_ctx* c, std::vector<DigestItem>& items);
+void digest_colblocks(int nD, int* TN, int* ncolblk);
+
+// ltjk_eri.cu
+int launch_pair_records(ltjk_ctx* c, const double* d_xyz, const int* d_atom, const int* d_l, const int* d_nprim,
+                        const int* d_poff, const double* d_exps, const double* d_coef, const int* d_int2ext);
+int launch_schwarz(ltjk_ctx* c, const int* lrange_host);
+int launch_eri_panels(ltjk_ctx* c, const Chunk& ch, int ra, int rb, int cb, int ck);
+int launch_eri_single(ltjk_ctx* c, int A, int B, int C, int D, int la, int lb, int lc, int ld, double* d_out);
+int launch_boys_debug(ltjk_ctx* c, int mmax, int n, const double* d_T, double* d_F);
+
+// ltjk_digest.cu
+int launch_digest(ltjk_ctx* c, const Chunk& ch, int nDp, bool doJ, bool doK);
+int launch_pack_densities(ltjk_ctx* c, int nD, int nDp, const double* D);
+int launch_unpack_results(ltjk_ctx* c, int nD, int nDp, double* J, double* K);
+int bench_dfma(ltjk_ctx* c, double* tflops);
+int bench_copy(ltjk_ctx* c, double* gbs);
+
+// ltjk_transform.cu
+int launch_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                            const double* eps_occ, const double* eps_vir, int nT, const double* T, int ntau,
+                            const double* tau_host, double* D_out);
+
+}  // namespace ltjk

@@ -1,0 +1,142 @@
+// ltjk_transform.cu -- step a4: Laplace pseudo-densities (Eqs. 13-15; Alg. 1 lines 5-7)
+//   D^{alpha,d} = (C_o e^{+eps_o tau_alpha}) T_d (C_v e^{-eps_v tau_alpha})^T
+// evaluated as two batched fp64 GEMMs per (alpha, d):
+//   W = [e^{(eps_i - eps_b) tau} T_d[i][b]] . C_v^T      (nocc x N)      -- the exponentials are fused into the load
+//   D = C_o . W                                          (N x N)
+// (nocc < nvir, so contracting the virtual index first is the cheaper order.)
+#include "ltjk_internal.h"
+
+namespace ltjk {
+
+__global__ void exp_factors_kernel(int nocc, int nvir, int ntau, const double* __restrict__ eo,
+                                   const double* __restrict__ ev, const double* __restrict__ tau,
+                                   double* __restrict__ fo, double* __restrict__ fv)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int n = nocc + nvir;
+    if (t >= ntau * n) return;
+    const int a = t / n, i = t % n;
+    if (i < nocc) fo[a * nocc + i] = exp(eo[i] * tau[a]);
+    else fv[a * nvir + (i - nocc)] = exp(-ev[i - nocc] * tau[a]);
+}
+
+// C[z] (M x Nn, row-major) = A[z] (M x K, row-major, optionally scaled sr[i]*sc[k]) . B
+//   TRANSB = true : B given as Bt (Nn x K row-major), i.e. C = A . Bt^T
+//   TRANSB = false: B (K x Nn row-major)
+// batch z = za * nzb + zb; A advances with (za,zb) as given by the strides.
+struct GemmArgs {
+    int M, Nn, K;
+    const double* A; long long sAa, sAb;
+    const double* B; long long sBa, sBb;
+    double* C; long long sCa, sCb;
+    const double* sr; long long ssr;     // row scale, per za (may be null)
+    const double* sc; long long ssc;     // column (k) scale, per za
+    int nzb;
+};
+
+template <bool TRANSB>
+__global__ void __launch_bounds__(256) gemm_kernel(const GemmArgs g)
+{
+    constexpr int BM = 64, BN = 64, BK = 16;
+    __shared__ double As[BK][BM + 2];
+    __shared__ double Bs[BK][BN + 2];
+    const int za = blockIdx.z / g.nzb, zb = blockIdx.z % g.nzb;
+    const double* __restrict__ A = g.A + za * g.sAa + zb * g.sAb;
+    const double* __restrict__ B = g.B + za * g.sBa + zb * g.sBb;
+    double* __restrict__ C = g.C + za * g.sCa + zb * g.sCb;
+    const double* sr = g.sr ? g.sr + za * g.ssr : nullptr;
+    const double* sc = g.sc ? g.sc + za * g.ssc : nullptr;
+    const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    double acc[4][4] = {};
+    for (int k0 = 0; k0 < g.K; k0 += BK) {
+        // A tile: 64 x 16, lanes along k (contiguous)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int k = tid & 15, m = (tid >> 4) + 16 * e;
+            const int gm = m0 + m, gk = k0 + k;
+            double v = 0.0;
+            if (gm < g.M && gk < g.K) {
+                v = A[(size_t)gm * g.K + gk];
+                if (sr) v *= sr[gm] * sc[gk];
+            }
+            As[k][m] = v;
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            double v = 0.0;
+            if (TRANSB) {
+                const int k = tid & 15, n = (tid >> 4) + 16 * e;
+                const int gn = n0 + n, gk = k0 + k;
+                if (gn < g.Nn && gk < g.K) v = B[(size_t)gn * g.K + gk];
+                Bs[k][n] = v;
+            } else {
+                const int n = tid & 63, k = (tid >> 6) + 4 * e;
+                const int gn = n0 + n, gk = k0 + k;
+                if (gn < g.Nn && gk < g.K) v = B[(size_t)gk * g.Nn + gn];
+                Bs[k][n] = v;
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < BK; ++k) {
+            double a[4], b[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) a[i] = As[k][ty * 4 + i];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = Bs[k][tx + 16 * j];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int gm = m0 + ty * 4 + i;
+        if (gm >= g.M) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int gn = n0 + tx + 16 * j;
+            if (gn < g.Nn) C[(size_t)gm * g.Nn + gn] = acc[i][j];
+        }
+    }
+}
+
+int launch_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                            const double* eps_occ, const double* eps_vir, int nT, const double* T, int ntau,
+                            const double* tau_host, double* D_out)
+{
+    const int N = c->nao;
+    double *tau = nullptr, *fo = nullptr, *fv = nullptr, *W = nullptr;
+    LTJK_CUDA(c, cudaMallocAsync(&tau, sizeof(double) * ntau, c->stream));
+    LTJK_CUDA(c, cudaMallocAsync(&fo, sizeof(double) * ntau * nocc, c->stream));
+    LTJK_CUDA(c, cudaMallocAsync(&fv, sizeof(double) * ntau * nvir, c->stream));
+    LTJK_CUDA(c, cudaMallocAsync(&W, sizeof(double) * (size_t)ntau * nT * nocc * N, c->stream));
+    LTJK_CUDA(c, cudaMemcpyAsync(tau, tau_host, sizeof(double) * ntau, cudaMemcpyHostToDevice, c->stream));
+    const int ne = ntau * (nocc + nvir);
+    exp_factors_kernel<<<(ne + 127) / 128, 128, 0, c->stream>>>(nocc, nvir, ntau, eps_occ, eps_vir, tau, fo, fv);
+    LTJK_CUDA(c, cudaGetLastError());
+    GemmArgs g1;   // W[a][d] = (fo[a] .* T[d] .* fv[a]) . C_vir^T
+    g1.M = nocc; g1.Nn = N; g1.K = nvir;
+    g1.A = T; g1.sAa = 0; g1.sAb = (long long)nocc * nvir;
+    g1.B = C_vir; g1.sBa = 0; g1.sBb = 0;
+    g1.C = W; g1.sCa = (long long)nT * nocc * N; g1.sCb = (long long)nocc * N;
+    g1.sr = fo; g1.ssr = nocc; g1.sc = fv; g1.ssc = nvir; g1.nzb = nT;
+    gemm_kernel<true><<<dim3((N + 63) / 64, (nocc + 63) / 64, ntau * nT), 256, 0, c->stream>>>(g1);
+    LTJK_CUDA(c, cudaGetLastError());
+    GemmArgs g2;   // D[a][d] = C_occ . W[a][d]
+    g2.M = N; g2.Nn = N; g2.K = nocc;
+    g2.A = C_occ; g2.sAa = 0; g2.sAb = 0;
+    g2.B = W; g2.sBa = (long long)nT * nocc * N; g2.sBb = (long long)nocc * N;
+    g2.C = D_out; g2.sCa = (long long)nT * N * N; g2.sCb = (long long)N * N;
+    g2.sr = nullptr; g2.ssr = 0; g2.sc = nullptr; g2.ssc = 0; g2.nzb = nT;
+    gemm_kernel<false><<<dim3((N + 63) / 64, (N + 63) / 64, ntau * nT), 256, 0, c->stream>>>(g2);
+    LTJK_CUDA(c, cudaGetLastError());
+    cudaFreeAsync(tau, c->stream); cudaFreeAsync(fo, c->stream); cudaFreeAsync(fv, c->stream); cudaFreeAsync(W, c->stream);
+    c->st_launches += 3;
+    return LTJK_OK;
+}
+
+}  // namespace ltjk

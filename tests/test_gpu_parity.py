@@ -1,0 +1,165 @@
+"""GPU parity tier: the CUDA path, called through the C ABI (ctypes binding), against the CPU oracle, element by
+element, on the same seeded inputs.  Bar (BASELINE.json north_star; reading A11): per output matrix X,
+max|X_gpu - X_ref| / max|X_ref| <= 1e-10 in fp64."""
+import itertools
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2607_05622_b200.inputs import SCHWARZ_TAU, custom_basis, make_workload, random_densities
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+def relerr(x, ref):
+    """A11: max-abs error normalised by the max-abs of the reference matrix (per matrix, worst over the batch)."""
+    x = np.asarray(x)
+    ref = np.asarray(ref)
+    if x.ndim == 2:
+        x, ref = x[None], ref[None]
+    num = np.abs(x - ref).reshape(x.shape[0], -1).max(1)
+    den = np.abs(ref).reshape(x.shape[0], -1).max(1)
+    return float((num / den).max())
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests (there is no CPU fallback)")
+    return torch
+
+
+def make_ctx(basis, tau=SCHWARZ_TAU, scratch=None):
+    from paper_2607_05622_b200 import ltjk
+    ctx = ltjk.Context(0)
+    if scratch is not None:
+        ctx.set_scratch_bytes(scratch)
+    ctx.set_basis(basis)
+    ctx.build_shell_pairs(tau)
+    return ctx
+
+
+def gpu_jk(torch, ctx, D):
+    Dd = torch.from_numpy(np.ascontiguousarray(D)).cuda()
+    J = torch.empty_like(Dd)
+    K = torch.empty_like(Dd)
+    ctx.jk_build(Dd, J, K)
+    torch.cuda.synchronize()
+    return J.cpu().numpy(), K.cpu().numpy()
+
+
+def test_boys_device_vs_oracle(torch_cuda, tiny):
+    ctx = make_ctx(tiny.basis)
+    T = np.array([0.0, 1e-9, 1e-3, 0.06, 0.0625, 0.5, 5.0, 20.0, 34.9, 35.93, 35.99999, 36.0, 36.1, 100.0, 1e3, 6e3])
+    for mmax in (0, 3, 8):
+        F = ctx.debug_boys(mmax, T)
+        ref = np.array([O.boys(mmax, t) for t in T])
+        assert np.all(np.abs(F - ref) <= 2e-14 * np.abs(ref))
+
+
+def test_eri_all_classes_vs_oracle(torch_cuda):
+    rng = np.random.default_rng(7)
+    xyz = rng.uniform(-1.5, 1.5, size=(4, 3))
+    xyz[3] = xyz[0]
+    shells = []
+    for ia in range(4):
+        shells.append([(l, [0.3 + 0.4 * ia + 0.2 * l, 1.1 + 0.3 * ia + 0.5 * l], [0.6, 0.4]) for l in range(3)])
+    b = custom_basis(xyz, shells)
+    ctx = make_ctx(b)
+    worst = 0.0
+    for la, lb, lc, ld in itertools.product(range(3), repeat=4):      # all 81 ordered classes through the hook
+        A, B, C, D = 0 * 3 + la, 1 * 3 + lb, 2 * 3 + lc, 3 * 3 + ld
+        out = ctx.debug_eri_quartet(b, A, B, C, D)
+        ref = O.eri_shell(b, A, B, C, D)
+        err = np.abs(out - ref).max() / np.abs(ref).max()
+        worst = max(worst, err)
+        assert err < 1e-12, ((la, lb, lc, ld), err)
+    assert worst < 1e-12
+
+
+def test_schwarz_vs_oracle(torch_cuda, small):
+    ctx = make_ctx(small.basis)
+    Q = ctx.get_schwarz()
+    Qr = O.schwarz(small.basis)
+    # Q^2 is the integral (ab|ab): absolute agreement at round-off of the largest one; Q itself (a square root, so
+    # ill-conditioned near zero) to 1e-10 relative wherever it matters for a 1e-12 product threshold
+    assert np.abs(Q ** 2 - Qr ** 2).max() <= 1e-13 * np.abs(Qr ** 2).max()
+    big = Qr > 1e-4
+    assert np.abs(Q[big] / Qr[big] - 1.0).max() <= 1e-10
+    assert np.allclose(Q, Q.T)
+
+
+def test_jk_tiny_vs_definition(torch_cuda, tiny):
+    """BASELINE gate: GPU vs the brute-force explicit-N^4 contraction (oracle O7) on the tiny config."""
+    b = tiny.basis
+    D = random_densities(b.nao, 3, seed=11)
+    ctx = make_ctx(b, tau=0.0)
+    J, K = gpu_jk(torch_cuda, ctx, D)
+    eri = O.eri_tensor(b)
+    Jr, Kr = O.jk_definition(eri, D)
+    assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
+    # non-symmetric K: the antisymmetric part must be there
+    assert np.abs(K - K.transpose(0, 2, 1)).max() > 1e-3 * np.abs(K).max()
+
+
+def test_jk_spd_vs_definition(torch_cuda, spd_basis):
+    """s, p and d shells (all 21 canonical classes, diagonal blocks included) against Eq. 17 literally."""
+    b = spd_basis
+    D = random_densities(b.nao, 5, seed=12)
+    ctx = make_ctx(b, tau=0.0)
+    J, K = gpu_jk(torch_cuda, ctx, D)
+    Jr, Kr = O.jk_definition(O.eri_tensor(b), D)
+    assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
+
+
+def test_jk_tiny_pseudo_densities_end_to_end(torch_cuda, tiny):
+    """Transform (a4) + J/K (a5-a9) on the tiny workload vs oracle O10 + O6."""
+    torch = torch_cuda
+    w = tiny
+    tau, wts, _, _ = (np.linspace(0.1, 3.0, w.ntau), None, None, None)
+    ctx = make_ctx(w.basis)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Dg = torch.empty((w.ntau, w.nT, w.nao, w.nao), dtype=torch.float64, device="cuda")
+    ctx.build_pseudo_densities(dev(w.C_occ), dev(w.C_vir), dev(w.eps_occ), dev(w.eps_vir), dev(w.T), tau, Dg)
+    torch.cuda.synchronize()
+    Dr = O.pseudo_densities_loops(w.C_occ, w.C_vir, w.eps_occ, w.eps_vir, w.T, tau)
+    assert relerr(Dg.cpu().numpy().reshape(-1, w.nao, w.nao), Dr.reshape(-1, w.nao, w.nao)) < 1e-12
+    D = Dr.reshape(-1, w.nao, w.nao)
+    J, K = gpu_jk(torch, ctx, D)
+    Jr, Kr, _ = O.jk_folded(w.basis, D, w.schwarz_tau)
+    assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
+
+
+@pytest.mark.parametrize("scratch", [None, 1 << 20])
+def test_jk_small_vs_folded(torch_cuda, small, scratch):
+    """160 AO, contracted s/p/d, ragged blocks; a small scratch forces many chunks per bra block pair."""
+    w = small
+    D = random_densities(w.nao, 5, seed=13)
+    ctx = make_ctx(w.basis, scratch=scratch)
+    J, K = gpu_jk(torch_cuda, ctx, D)
+    Jr, Kr, kept = O.jk_folded(w.basis, D, w.schwarz_tau)
+    assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
+    # J-only and K-only entry points give the same matrices
+    torch = torch_cuda
+    Dd = torch.from_numpy(D).cuda()
+    J2 = torch.empty_like(Dd)
+    ctx.jk_build(Dd, J2, None)
+    K2 = torch.empty_like(Dd)
+    ctx.jk_build(Dd, None, K2)
+    torch.cuda.synchronize()
+    assert relerr(J2.cpu().numpy(), Jr) < TOL and relerr(K2.cpu().numpy(), Kr) < TOL
+
+
+def test_jk_host_entry_matches_device_entry(torch_cuda, tiny):
+    D = random_densities(tiny.nao, 40, seed=14)       # 40 densities: two column blocks of the digestion
+    ctx = make_ctx(tiny.basis)
+    J, K = gpu_jk(torch_cuda, ctx, D)
+    Jh, Kh = ctx.jk_build_host(D)
+    assert np.array_equal(np.isfinite(Jh), np.ones_like(Jh, dtype=bool))
+    assert relerr(Jh, J) < 1e-13 and relerr(Kh, K) < 1e-13
+    Jr, Kr, _ = O.jk_folded(tiny.basis, D, tiny.schwarz_tau)
+    assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
