@@ -100,6 +100,14 @@ int ltjk_jk_build(ltjk_ctx* ctx, int nD, const double* D, double* J, double* K);
  * synchronises.  This is the end-to-end entry bench.py times as "e2e". */
 int ltjk_jk_build_host(ltjk_ctx* ctx, int nD, const double* D_host, double* J_host, double* K_host);
 
+/* One whole Laplace sweep with HOST buffers (steps a4-a9 end to end): copies C_occ[N][nocc], C_vir[N][nvir],
+ * eps_occ, eps_vir, T[nT][nocc][nvir] and tau[ntau] to the device, builds the ntau*nT pseudo-densities
+ * (Eq. 15), builds J and K for all of them (Eq. 17), copies J_host and K_host
+ * [ntau*nT][N][N] back (either may be NULL) and synchronises.  Pinned host memory makes the copies asynchronous. */
+int ltjk_sweep_host(ltjk_ctx* ctx, int nocc, int nvir, const double* C_occ_host, const double* C_vir_host,
+                    const double* eps_occ_host, const double* eps_vir_host, int nT, const double* T_host, int ntau,
+                    const double* tau_host, double* J_host, double* K_host);
+
 /* Statistics of the last ltjk_jk_build on this context (HOST outputs, any may be NULL):
  *   n_launches    kernels launched
  *   eri_quartets  contracted shell quartets evaluated (4-fold unique: A>=B, C>=D, all bra x ket)

@@ -40,7 +40,7 @@ void free_tables(ltjk_ctx* c)
     double* boys = t.boys;
     t = DevTables();
     t.boys = boys;
-    c->d_items = nullptr; c->d_panel = nullptr; c->panel_cap = 0; c->n_items = 0;
+    c->d_items = nullptr; c->d_panel = nullptr; c->panel_cap = 0; c->panel_half = 0; c->n_items = 0;
     c->have_pairs = false;
 }
 
@@ -65,7 +65,7 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
     for (int rIJ = 0; rIJ < npair; ++rIJ) {
         const int I = c->pair_I[rIJ], J = c->pair_J[rIJ];
         const int nI = c->blk_nao[I], nJ = c->blk_nao[J];
-        const long long cap = std::max<long long>(c->panel_cap / ((long long)nI * nJ), 1);
+        const long long cap = std::max<long long>(c->panel_half / ((long long)nI * nJ), 1);
         int r0 = 0;
         while (r0 <= rIJ) {
             int r1 = r0 + 1;
@@ -84,6 +84,7 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
                     items.push_back(DigestItem{1, 0, (unsigned short)rt, r, 0, 1});
             }
             ch.nitemsJ = (int)((long long)items.size() - ch.item0);
+            const size_t k_first = items.size();
             // ---- K views 2,3: runs of consecutive ranks with the same K (L consecutive by construction)
             for (int ra = r0; ra < r1;) {
                 const int K = c->pair_I[ra];
@@ -121,6 +122,11 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
                 ks.clear();
             }
             ch.nitemsK = (int)((long long)items.size() - ch.item0) - ch.nitemsJ;
+            // longest runs first: shortens the tail of each launch
+            auto longer = [](const DigestItem& a, const DigestItem& b) { return a.count > b.count; };
+            std::stable_sort(items.begin() + ch.item0, items.begin() + k_first, longer);
+            std::stable_sort(items.begin() + k_first, items.end(), longer);
+            ch.buf = (int)(c->chunks.size() & 1);
             c->chunks.push_back(ch);
             r0 = r1;
         }
@@ -144,6 +150,13 @@ int ltjk_create(ltjk_ctx** out, int device, void* cuda_stream)
     if (!c) return LTJK_ENOMEM;
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
+    if (cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return LTJK_ECUDA; }
+    c->eri_stream = c->own_stream;
+    for (int i = 0; i < 2; ++i) {
+        cudaEventCreateWithFlags(&c->ev_eri[i], cudaEventDisableTiming);
+        cudaEventCreateWithFlags(&c->ev_dig[i], cudaEventDisableTiming);
+    }
+    cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming);
     std::vector<double> tab = make_boys_table(kBoysNT, kBoysNM);
     if (cudaMalloc(&c->t.boys, sizeof(double) * tab.size()) != cudaSuccess ||
         cudaMemcpy(c->t.boys, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
@@ -162,6 +175,10 @@ int ltjk_destroy(ltjk_ctx* c)
     free_tables(c);
     free_work(c);
     if (c->t.boys) cudaFree(c->t.boys);
+    for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_eri[i]); cudaEventDestroy(c->ev_dig[i]); }
+    cudaEventDestroy(c->ev_start);
+    cudaStreamSynchronize(c->own_stream);
+    cudaStreamDestroy(c->own_stream);
     delete c;
     return LTJK_OK;
 }

@@ -123,10 +123,11 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     // ---- panel staging ring: L2-sized by default, never below one panel
     size_t freeb = 0, totb = 0;
     LTJK_CUDA(c, cudaMemGetInfo(&freeb, &totb));
-    long long bytes = c->scratch_bytes > 0 ? c->scratch_bytes : (64ll << 20);
+    long long bytes = c->scratch_bytes > 0 ? c->scratch_bytes : (96ll << 20);
     bytes = std::min<long long>(bytes, (long long)(0.6 * (double)freeb));
     long long total = c->koff[npair] * c->koff[npair];      // never need more than everything at once
-    c->panel_cap = std::max<long long>(std::min<long long>(bytes / 8, total), maxpanel);
+    c->panel_half = std::max<long long>(std::min<long long>(bytes / 16, total), maxpanel);
+    c->panel_cap = 2 * c->panel_half;
     LTJK_CUDA(c, cudaMalloc(&c->d_panel, sizeof(double) * c->panel_cap));
 
     std::vector<DigestItem> items;
@@ -187,8 +188,18 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
         }
         cls_start[6] = r;
     }
+    // Two-stream pipeline over the two halves of the panel ring: ERI(c+1) on eri_stream overlaps digest(c) on
+    // the context stream (both are DFMA-bound; the overlap fills the tail of each launch).  Timing mode serialises
+    // the two phases on the context stream so that per-phase durations are those of the kernels alone.
+    c->eri_stream = c->timing ? c->stream : c->own_stream;
+    if (!c->timing) {
+        LTJK_CUDA(c, cudaEventRecord(c->ev_start, c->stream));          // everything enqueued before this build
+        LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_start, 0));
+    }
+    long long ci = 0;
     for (const Chunk& ch : c->chunks) {
         const int cb = pair_class(c->blk_l[ch.I], c->blk_l[ch.J]);
+        if (!c->timing && ci >= 2) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[ch.buf], 0));
         if (c->timing) cudaEventRecord(e0, c->stream);
         for (int ck = 0; ck <= cb; ++ck) {
             const int ra = std::max(ch.r0, cls_start[ck]), rb = std::min(ch.r1, cls_start[ck + 1]);
@@ -196,7 +207,13 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
             if ((rc = launch_eri_panels(c, ch, ra, rb, cb, ck))) return rc;
         }
         if (c->timing) cudaEventRecord(e1, c->stream);
+        else {
+            LTJK_CUDA(c, cudaEventRecord(c->ev_eri[ch.buf], c->eri_stream));
+            LTJK_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_eri[ch.buf], 0));
+        }
         if ((rc = launch_digest(c, ch, nDp, J != nullptr, K != nullptr))) return rc;
+        if (!c->timing) LTJK_CUDA(c, cudaEventRecord(c->ev_dig[ch.buf], c->stream));
+        ++ci;
         if (c->timing) {
             cudaEventRecord(e2, c->stream);
             cudaEventSynchronize(e2);
@@ -253,6 +270,46 @@ int ltjk_build_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C
         return set_err(c, LTJK_EINVAL, "build_pseudo_densities: bad arguments");
     cudaSetDevice(c->device);
     return launch_pseudo_densities(c, nocc, nvir, C_occ, C_vir, eps_occ, eps_vir, nT, T, ntau, tau_host, D_out);
+}
+
+int ltjk_sweep_host(ltjk_ctx* c, int nocc, int nvir, const double* C_occ_host, const double* C_vir_host,
+                    const double* eps_occ_host, const double* eps_vir_host, int nT, const double* T_host, int ntau,
+                    const double* tau_host, double* J_host, double* K_host)
+{
+    if (!c) return LTJK_EINVAL;
+    if (!c->have_pairs) return set_err(c, LTJK_ENOBASIS, "sweep_host: shell pairs not built");
+    if (nocc <= 0 || nvir <= 0 || nT <= 0 || ntau <= 0 || !C_occ_host || !C_vir_host || !eps_occ_host || !eps_vir_host ||
+        !T_host || !tau_host || (!J_host && !K_host))
+        return set_err(c, LTJK_EINVAL, "sweep_host: bad arguments");
+    cudaSetDevice(c->device);
+    const long long N = c->nao, nD = (long long)ntau * nT;
+    const long long need = nD * N * N;
+    if (need > c->host_cap) {
+        double** bufs[] = {&c->hD, &c->hJ, &c->hK};
+        for (double** b : bufs) {
+            if (*b) { cudaFree(*b); *b = nullptr; }
+            c->host_cap = 0;
+            LTJK_CUDA(c, cudaMalloc((void**)b, sizeof(double) * need));
+        }
+        c->host_cap = need;
+    }
+    const size_t nin = (size_t)N * nocc + (size_t)N * nvir + nocc + nvir + (size_t)nT * nocc * nvir;
+    double* in = nullptr;
+    LTJK_CUDA(c, cudaMallocAsync(&in, sizeof(double) * nin, c->stream));
+    double *dCo = in, *dCv = dCo + (size_t)N * nocc, *deo = dCv + (size_t)N * nvir, *dev = deo + nocc, *dT = dev + nvir;
+    LTJK_CUDA(c, cudaMemcpyAsync(dCo, C_occ_host, sizeof(double) * N * nocc, cudaMemcpyHostToDevice, c->stream));
+    LTJK_CUDA(c, cudaMemcpyAsync(dCv, C_vir_host, sizeof(double) * N * nvir, cudaMemcpyHostToDevice, c->stream));
+    LTJK_CUDA(c, cudaMemcpyAsync(deo, eps_occ_host, sizeof(double) * nocc, cudaMemcpyHostToDevice, c->stream));
+    LTJK_CUDA(c, cudaMemcpyAsync(dev, eps_vir_host, sizeof(double) * nvir, cudaMemcpyHostToDevice, c->stream));
+    LTJK_CUDA(c, cudaMemcpyAsync(dT, T_host, sizeof(double) * (size_t)nT * nocc * nvir, cudaMemcpyHostToDevice, c->stream));
+    int rc = launch_pseudo_densities(c, nocc, nvir, dCo, dCv, deo, dev, nT, dT, ntau, tau_host, c->hD);
+    if (!rc) rc = ltjk_jk_build(c, (int)nD, c->hD, J_host ? c->hJ : nullptr, K_host ? c->hK : nullptr);
+    cudaFreeAsync(in, c->stream);
+    if (rc) return rc;
+    if (J_host) LTJK_CUDA(c, cudaMemcpyAsync(J_host, c->hJ, sizeof(double) * need, cudaMemcpyDeviceToHost, c->stream));
+    if (K_host) LTJK_CUDA(c, cudaMemcpyAsync(K_host, c->hK, sizeof(double) * need, cudaMemcpyDeviceToHost, c->stream));
+    LTJK_CUDA(c, cudaStreamSynchronize(c->stream));
+    return LTJK_OK;
 }
 
 int ltjk_get_stats(const ltjk_ctx* c, long long* n_launches, long long* eri_quartets, double* digest_flops,

@@ -224,7 +224,7 @@ int launch_digest(ltjk_ctx* c, const Chunk& ch, int nDp, bool doJ, bool doK)
     const int nitems = (doJ ? ch.nitemsJ : 0) + (doK ? ch.nitemsK : 0);
     if (nitems == 0) return LTJK_OK;
     DigestArgs g;
-    g.t = c->t; g.items = c->d_items + first; g.panel = c->d_panel;
+    g.t = c->t; g.items = c->d_items + first; g.panel = c->d_panel + (size_t)ch.buf * c->panel_half;
     g.Dt = c->Dt; g.Dst = c->Dst; g.Jt = c->Jt; g.Kt = c->Kt;
     g.I = ch.I; g.J = ch.J; g.r0 = ch.r0; g.nDp = nDp;
     int TN, nb;

@@ -92,7 +92,8 @@ struct EriArgs {
 };
 
 template <int LA, int LB, int LC, int LD>
-__global__ void __launch_bounds__(64) eri_panel_kernel(const EriArgs g)
+// (64,4): without a min-blocks hint ptxas drops the heavy classes to 32 registers and spills ~80 KB per thread
+__global__ void __launch_bounds__(64, 4) eri_panel_kernel(const EriArgs g)
 {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int r = g.ra + (int)(t / g.qn);
@@ -145,7 +146,7 @@ static int launch_cls(ltjk_ctx* c, const EriArgs& g)
     if constexpr (CK <= CB) {
         const long long nthr = (long long)(g.rb - g.ra) * g.qn;
         const int bs = 64;
-        eri_panel_kernel<la[CB], lb[CB], la[CK], lb[CK]><<<(unsigned)((nthr + bs - 1) / bs), bs, 0, c->stream>>>(g);
+        eri_panel_kernel<la[CB], lb[CB], la[CK], lb[CK]><<<(unsigned)((nthr + bs - 1) / bs), bs, 0, c->eri_stream>>>(g);
         LTJK_CUDA(c, cudaGetLastError());
         return LTJK_OK;
     } else {
@@ -175,7 +176,7 @@ int launch_eri_panels(ltjk_ctx* c, const Chunk& ch, int ra, int rb, int cb, int 
     g.mJ = c->max_nsh_l[kClsLb[cb]]; g.mK = c->max_nsh_l[kClsLa[ck]]; g.mL = c->max_nsh_l[kClsLb[ck]];
     g.qn = mI * g.mJ * g.mK * g.mL;
     g.tau = c->tau;
-    g.panel = c->d_panel;
+    g.panel = c->d_panel + (size_t)ch.buf * c->panel_half;
     c->st_launches++;
     switch (cb) {
     case 0: return launch_cls_k<0>(c, ck, g);

@@ -45,6 +45,7 @@ struct Chunk {
     int r0, r1;             // ket ranks [r0, r1)
     long long item0;        // first digest item: nitemsJ J-view items, then nitemsK K-view items
     int nitemsJ, nitemsK;
+    int buf;                // which half of the panel ring (chunks alternate)
 };
 
 }  // namespace ltjk
@@ -78,7 +79,11 @@ struct ltjk_ctx {
     ltjk::DigestItem* d_items = nullptr;
     long long n_items = 0;
     double* d_panel = nullptr;            // integral panel staging ring (L2-sized)
-    long long panel_cap = 0;              // doubles
+    long long panel_cap = 0;              // doubles (both halves)
+    long long panel_half = 0;             // doubles per half: chunk c lives in half c&1 (ERI of c+1 overlaps digest of c)
+    cudaStream_t eri_stream = nullptr;    // stream of the ERI kernels (== stream when timing serialises the phases)
+    cudaStream_t own_stream = nullptr;
+    cudaEvent_t ev_eri[2] = {nullptr, nullptr}, ev_dig[2] = {nullptr, nullptr}, ev_start = nullptr;
 
     // per-build work buffers (grown on demand): density-fastest internal layouts [N][N][nDp]
     double *Dt = nullptr, *Dst = nullptr, *Jt = nullptr, *Kt = nullptr;

@@ -23,7 +23,7 @@ ERRORS = {0: "LTJK_OK", -1: "LTJK_EINVAL", -2: "LTJK_ENOBASIS", -3: "LTJK_ECUDA"
 EXPORTS = [
     "ltjk_create", "ltjk_destroy", "ltjk_last_error", "ltjk_set_scratch_bytes", "ltjk_set_basis", "ltjk_get_nao",
     "ltjk_build_shell_pairs", "ltjk_get_schwarz", "ltjk_laplace_quadrature", "ltjk_build_pseudo_densities",
-    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_get_stats", "ltjk_set_timing", "ltjk_debug_eri_quartet",
+    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_get_stats", "ltjk_set_timing", "ltjk_debug_eri_quartet",
     "ltjk_debug_boys", "ltjk_bench_dfma_peak", "ltjk_bench_copy_peak",
 ]
 
@@ -178,6 +178,21 @@ class Context:
             K = np.empty(tuple(D.shape))
         self._chk(self.lib.ltjk_jk_build_host(self._h, ctypes.c_int(D.shape[0]), hp(D), hp(J), hp(K)))
         return J, K
+
+    def sweep_host(self, C_occ, C_vir, eps_occ, eps_vir, T, tau, J=None, K=None):
+        """ltjk_sweep_host: host buffers (numpy float64 C-contiguous, or pinned torch CPU tensors) in and out."""
+        def hp(a):
+            if a is None:
+                return ctypes.c_void_p(0)
+            if isinstance(a, np.ndarray):
+                assert a.dtype == np.float64 and a.flags.c_contiguous
+                return ctypes.c_void_p(a.ctypes.data)
+            assert a.dtype.is_floating_point and a.is_contiguous() and not a.is_cuda
+            return ctypes.c_void_p(a.data_ptr())
+        tau = np.ascontiguousarray(tau, dtype=np.float64)
+        self._chk(self.lib.ltjk_sweep_host(
+            self._h, ctypes.c_int(C_occ.shape[1]), ctypes.c_int(C_vir.shape[1]), hp(C_occ), hp(C_vir), hp(eps_occ),
+            hp(eps_vir), ctypes.c_int(T.shape[0]), hp(T), ctypes.c_int(tau.shape[0]), _d(tau), hp(J), hp(K)))
 
     def get_stats(self) -> dict:
         nl = ctypes.c_longlong(0)
