@@ -182,8 +182,8 @@ def main():
     N, nD = w.nao, w.nD
     # Multi-GPU: the path shards over independent problems -- every rank runs its own
     # sweep on its own batch of n_T amplitude sets (same molecule, rank-seeded T); no data-path collective.
-    rng = np.random.default_rng(1000 + rank)
-    T_host = w.T if rank == 0 else 1e-2 * rng.standard_normal(w.T.shape)
+    from paper_2607_05622_b200.dist import max_over_ranks, rank_amplitudes, whole_job_builds_per_s
+    T_host = rank_amplitudes(w, rank)
 
     stream = torch.cuda.current_stream()
     ctx = ltjk.Context(local, stream)
@@ -226,12 +226,9 @@ def main():
     ms = e0.elapsed_time(e1)
     launches_jk = ctx.get_stats()["n_launches"]
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, "cuda")
     ms_per_step = ms / args.steps
-    value = world * nD / (ms_per_step * 1e-3)
+    value = whole_job_builds_per_s(nD, world, ms_per_step)
 
     # ---- e2e: the same sweep through the C ABI with HOST (pinned) buffers
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -248,10 +245,7 @@ def main():
     e1.record(stream)
     barrier()
     ms_e2e = e0.elapsed_time(e1) / n_e2e
-    if world > 1:
-        t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
+    ms_e2e = max_over_ranks(ms_e2e, "cuda")
     h2d = 8 * (hCo.numel() + hCv.numel() + heo.numel() + hev.numel() + hT.numel())
     d2h = 8 * (hJ.numel() + hK.numel())
     assert torch.equal(hK, K.cpu()) or float((hK - K.cpu()).abs().max()) < 1e-9 * float(K.abs().max())
@@ -292,7 +286,7 @@ def main():
                       "setup_outside_timed_region": "basis upload, shell pairs, Schwarz, work lists (geometry-frozen)",
                       "laplace_grid": "library minimax" if wts is not None else "placeholder linspace (cost is value-independent)"},
            "clocks": clocks,
-           "e2e": {"value": world * nD / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+           "e2e": {"value": whole_job_builds_per_s(nD, world, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                    "ms_per_step": ms_e2e},
            "gpu_launches": int((launches_jk + 3) * args.steps),
            "roofline": roofline, "cpu_baseline": cpu}

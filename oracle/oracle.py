@@ -172,12 +172,16 @@ def pseudo_densities_loops(C_occ, C_vir, eps_occ, eps_vir, T, tau) -> np.ndarray
 # ---------------------------------------------------------------------------------------------------------
 # O9 minimax exponential-sum approximation of 1/x on [xmin, xmax] (Eq. (11), refs 18-19 of the paper):
 # minimise max_x |1/x - sum_a w_a exp(-x tau_a)|.  Solved on [1, R], R = xmax/xmin, then tau = tau^/xmin,
-# w = w^/xmin.  Remez exchange on the 2k+1 alternation points with Newton on the 2k parameters + level,
-# started from the trapezoid rule for 1/x = int exp(-x e^s) e^s ds; 120-digit arithmetic (mpmath) so that the
-# oracle's grid is converged far beyond fp64.
+# w = w^/xmin.  Remez exchange: Newton on E(x_j) = (-1)^j delta for the 2k parameters + level at the 2k+1
+# alternation points, then every interior point moves to the neighbouring extremum of E; 80-digit arithmetic
+# (mpmath) so that the oracle's grid is converged far beyond fp64.  Start: on a WIDER interval [1, R0] (well
+# conditioned) a least-squares fit (scipy, a library routine as a step) from the trapezoid rule for
+# 1/x = int exp(-x e^s) e^s ds, accepted only if its error curve already has 2k+1 alternating extrema; then
+# R0 -> R in geometric steps, each a full Remez solve started from the previous one.
 def laplace_minimax(xmin: float, xmax: float, k: int, verbose: bool = False):
     import mpmath as mp
-    mp.mp.dps = 120   # the Newton matrices are very ill-conditioned: pivots far below 1e-50 occur
+    from scipy.optimize import least_squares
+    mp.mp.dps = 80
     R = mp.mpf(xmax) / mp.mpf(xmin)
 
     def err(x, tau, w):
@@ -188,13 +192,16 @@ def laplace_minimax(xmin: float, xmax: float, k: int, verbose: bool = False):
 
     def remez(Rc, tau, w, xs, iters=60):
         delta = mp.mpf(0)
+        n = 2 * k + 1
         for it in range(iters):
-            # Newton on E(x_j) - (-1)^j delta = 0 for the unknowns (tau, w, delta)
-            for nit in range(60):
-                Fv = mp.matrix(2 * k + 1, 1)
-                Jm = mp.matrix(2 * k + 1, 2 * k + 1)
+            for nit in range(80):
+                Fv = mp.matrix(n, 1)
                 for j, x in enumerate(xs):
                     Fv[j] = err(x, tau, w) - (-1) ** j * delta
+                if nit > 0 and max(abs(v) for v in Fv) < mp.mpf(10) ** (-30) * abs(delta):
+                    break
+                Jm = mp.matrix(n, n)
+                for j, x in enumerate(xs):
                     for a in range(k):
                         ex = mp.e ** (-x * tau[a])
                         Jm[j, a] = w[a] * x * ex
@@ -207,8 +214,8 @@ def laplace_minimax(xmin: float, xmax: float, k: int, verbose: bool = False):
                 tau = [tau[a] + step * dx[a] for a in range(k)]
                 w = [w[a] + step * dx[k + a] for a in range(k)]
                 delta = delta + step * dx[2 * k]
-                if max(abs(v) for v in dx) < mp.mpf(10) ** (-40):
-                    break
+            else:
+                raise RuntimeError("laplace_minimax: Newton did not converge")
             # exchange: move every interior point to the local extremum of E next to it; endpoints stay
             new = [mp.mpf(1)]
             for j in range(1, 2 * k):
@@ -218,50 +225,64 @@ def laplace_minimax(xmin: float, xmax: float, k: int, verbose: bool = False):
                 vals = [err(x, tau, w) * sgn for x in grid]
                 m = max(range(41), key=lambda t: vals[t])
                 a_, b_ = grid[max(m - 1, 0)], grid[min(m + 1, 40)]
-                try:
-                    xr = mp.findroot(lambda x: derr(x, tau, w), (a_, b_), solver="illinois",
-                                     tol=mp.mpf(10) ** (-40))
-                    if not (a_ <= xr <= b_):
-                        xr = grid[m]
-                except Exception:
-                    xr = grid[m]
+                xr = grid[m]
+                if sgn * derr(a_, tau, w) > 0 and sgn * derr(b_, tau, w) < 0:
+                    for _ in range(200):            # bisection on the sign of E'
+                        mid = (a_ + b_) / 2
+                        if sgn * derr(mid, tau, w) > 0:
+                            a_ = mid
+                        else:
+                            b_ = mid
+                    xr = (a_ + b_) / 2
                 new.append(xr)
             new.append(Rc)
-            shift = max(abs(a - b) for a, b in zip(new, xs))
+            shift = max(abs(a - b) / b for a, b in zip(new, xs))
             xs = new
             if verbose:
                 print("remez R=%s it=%d delta=%s shift=%s" % (mp.nstr(Rc, 6), it, mp.nstr(delta, 8), mp.nstr(shift, 5)))
-            if shift < mp.mpf(10) ** (-25):
-                break
-        return tau, w, delta, xs
+            if shift < mp.mpf(10) ** (-20):
+                return tau, w, delta, xs
+        raise RuntimeError("laplace_minimax: exchange did not converge")
 
-    # Start: on a WIDER interval [1, R0] (well conditioned in fp64) fit by variable-projection least squares
-    # from the trapezoid rule for 1/x = int exp(-x e^s) e^s ds (library routines as steps), then walk R0 -> R
-    # in geometric steps, each a full Remez solve started from the previous one.
-    from scipy.optimize import least_squares
-    R0 = max(float(R), 10.0 ** (k / 3.0))
-    hh = (np.log(R0) + 5.5) / k
-    t0 = np.exp(-np.log(R0) - 2.5 + hh * (np.arange(k) + 0.5))
-    xg = np.exp(np.linspace(0.0, np.log(R0), 600))
+    def ls_start(R0):
+        n = 1500
+        hh = (np.log(R0) + 5.5) / k
+        s0 = -np.log(R0) - 2.5 + hh * (np.arange(k) + 0.5)
+        p0 = np.concatenate([s0, np.log(hh) + s0])
+        xg = np.exp(np.linspace(0.0, np.log(R0), n))
 
-    def solve_w(lt):
-        A = np.exp(-xg[:, None] * np.exp(lt)[None, :])
-        ww, *_ = np.linalg.lstsq(A, 1.0 / xg, rcond=None)
-        return A, ww
+        def res(p):
+            return 1.0 / xg - (np.exp(p[k:])[None, :] * np.exp(-xg[:, None] * np.exp(p[:k])[None, :])).sum(1)
 
-    sol = least_squares(lambda lt: solve_w(lt)[0] @ solve_w(lt)[1] - 1.0 / xg, np.log(t0), method="trf",
-                        xtol=1e-15, ftol=1e-15, gtol=1e-15, max_nfev=5000)
-    _, w0 = solve_w(sol.x)
-    order = np.argsort(sol.x)
-    tau = [mp.mpf(float(v)) for v in np.exp(sol.x[order])]
-    w = [mp.mpf(float(v)) for v in w0[order]]
-    if min(w) <= 0:
-        raise RuntimeError("laplace_minimax: least-squares start has a non-positive weight")
+        def jac(p):
+            t, ww = np.exp(p[:k]), np.exp(p[k:])
+            ex = np.exp(-xg[:, None] * t[None, :])
+            return np.concatenate([ww * t * xg[:, None] * ex, -ww * ex], axis=1)
+
+        with np.errstate(all="ignore"):
+            sol = least_squares(res, p0, jac=jac, method="lm", xtol=1e-15, ftol=1e-15, gtol=1e-15, max_nfev=20000)
+        E = res(sol.x)
+        idx = [0] + [i for i in range(1, n - 1) if (E[i] - E[i - 1]) * (E[i + 1] - E[i]) < 0] + [n - 1]
+        sg = np.sign(E[idx])
+        ok = len(idx) == 2 * k + 1 and bool(np.all(sg[1:] * sg[:-1] < 0)) and E[0] > 0
+        order = np.argsort(sol.x[:k])
+        return ok, np.exp(sol.x[:k])[order], np.exp(sol.x[k:])[order], xg[idx]
+
+    for c in (3.0, 2.6, 3.2, 2.8, 3.4, 2.4, 3.6, 2.2):
+        R0 = max(float(R), 10.0 ** (k / c))
+        ok, t0, w0, x0 = ls_start(R0)
+        if ok:
+            break
+    else:
+        raise RuntimeError("laplace_minimax: no least-squares start with 2k+1 alternating extrema")
+    tau = [mp.mpf(float(v)) for v in t0]
+    w = [mp.mpf(float(v)) for v in w0]
+    xs = [mp.mpf(float(v)) for v in x0]
+    xs[0], xs[-1] = mp.mpf(1), mp.mpf(R0)
     Rc = mp.mpf(R0)
-    xs = [Rc ** ((1 - mp.cos(mp.pi * j / (2 * k))) / 2) for j in range(2 * k + 1)]
     tau, w, delta, xs = remez(Rc, tau, w, xs)
     while Rc > R:
-        Rn = max(R, Rc / mp.mpf("1.3"))
+        Rn = max(R, Rc / mp.mpf("1.25"))
         xs = [Rn ** (mp.log(x) / mp.log(Rc)) for x in xs]
         Rc = Rn
         tau, w, delta, xs = remez(Rc, tau, w, xs)

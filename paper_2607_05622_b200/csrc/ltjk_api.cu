@@ -35,12 +35,12 @@ void free_tables(ltjk_ctx* c)
 {
     DevTables& t = c->t;
     void* ptrs[] = {t.pair_rec, t.schwarz, t.sh_ao, t.blk_sh0, t.blk_nsh, t.blk_ao0, t.blk_nao, t.pair_I, t.pair_J,
-                    t.koff, t.rank_of, t.ao_perm, c->d_items, c->d_panel};
+                    t.koff, t.rank_of, t.ao_perm, c->d_items, c->d_subs, c->d_panel};
     for (void* p : ptrs) if (p) cudaFree(p);
     double* boys = t.boys;
     t = DevTables();
     t.boys = boys;
-    c->d_items = nullptr; c->d_panel = nullptr; c->panel_cap = 0; c->panel_half = 0; c->n_items = 0;
+    c->d_items = nullptr; c->d_subs = nullptr; c->d_panel = nullptr; c->panel_cap = 0; c->panel_half = 0; c->n_items = 0;
     c->have_pairs = false;
 }
 
@@ -54,37 +54,87 @@ void free_work(ltjk_ctx* c)
 
 static inline int pair_class(int la, int lb) { return la * (la + 1) / 2 + lb; }
 
-// Build chunks (bra block pair x a range of ket ranks that fits the panel ring) and their digest items.
+// Build the geometry-frozen work lists: sub-chunks (bra block pair x a run of ket ranks), groups of sub-chunks that
+// fill one half of the panel ring, and the digestion items of every group.
 void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
 {
     const int nblk = (int)c->blk_nao.size(), npair = (int)c->pair_I.size();
-    c->chunks.clear();
+    c->subs.clear();
+    c->groups.clear();
     items.clear();
     auto rowtiles = [](int rows) { return (rows + 63) / 64; };
+    auto cls_of = [&](int r) { return pair_class(c->blk_l[c->pair_I[r]], c->blk_l[c->pair_J[r]]); };
+    {
+        int r = 0;
+        for (int cls = 0; cls < 6; ++cls) {
+            c->cls_start[cls] = r;
+            while (r < npair && cls_of(r) == cls) ++r;
+        }
+        c->cls_start[6] = r;
+    }
     std::vector<std::vector<int>> byL(nblk);
+    Group g;
+    bool open = false;
+    long long used = 0;                                   // doubles used in the current ring half
+    size_t j_first = 0;
+    std::vector<DigestItem> jitems, kitems;
+    auto close_group = [&]() {
+        if (!open) return;
+        auto longer = [](const DigestItem& a, const DigestItem& b) { return a.count > b.count; };
+        std::stable_sort(jitems.begin(), jitems.end(), longer);      // longest runs first: shorter launch tail
+        std::stable_sort(kitems.begin(), kitems.end(), longer);
+        g.item0 = (long long)items.size();
+        g.nitemsJ = (int)jitems.size(); g.nitemsK = (int)kitems.size();
+        items.insert(items.end(), jitems.begin(), jitems.end());
+        items.insert(items.end(), kitems.begin(), kitems.end());
+        jitems.clear(); kitems.clear();
+        g.buf = (int)(c->groups.size() & 1);
+        c->groups.push_back(g);
+        open = false;
+    };
+    (void)j_first;
     for (int rIJ = 0; rIJ < npair; ++rIJ) {
         const int I = c->pair_I[rIJ], J = c->pair_J[rIJ];
         const int nI = c->blk_nao[I], nJ = c->blk_nao[J];
-        const long long cap = std::max<long long>(c->panel_half / ((long long)nI * nJ), 1);
+        const long long nIJ = (long long)nI * nJ;
+        const int cb = cls_of(rIJ);
         int r0 = 0;
         while (r0 <= rIJ) {
+            if (open && (g.cb != cb || g.nsub >= 60000 || used + nIJ * (c->koff[r0 + 1] - c->koff[r0]) > c->panel_half))
+                close_group();
+            if (!open) {
+                g = Group();
+                g.sub0 = (int)c->subs.size(); g.nsub = 0; g.cb = cb; g.nquartets = 0; g.nints = 0.0;
+                for (int k = 0; k < 6; ++k) g.maxkets[k] = 0;
+                used = 0;
+                open = true;
+            }
             int r1 = r0 + 1;
-            while (r1 <= rIJ && c->koff[r1 + 1] - c->koff[r0] <= cap) ++r1;
-            Chunk ch;
-            ch.I = I; ch.J = J; ch.rIJ = rIJ; ch.r0 = r0; ch.r1 = r1; ch.item0 = (long long)items.size();
+            while (r1 <= rIJ && used + nIJ * (c->koff[r1 + 1] - c->koff[r0]) <= c->panel_half) ++r1;
+            SubChunk sc;
+            sc.I = I; sc.J = J; sc.rIJ = rIJ; sc.r0 = r0; sc.r1 = r1; sc.pad = 0; sc.base = used;
+            const int sub = (int)c->subs.size();
+            c->subs.push_back(sc);
+            g.nsub++;
+            used += nIJ * (c->koff[r1] - c->koff[r0]);
+            g.nints += (double)nIJ * (double)(c->koff[r1] - c->koff[r0]);
+            for (int k = 0; k < 6; ++k) {
+                const int a = std::max(r0, c->cls_start[k]), b = std::min(r1, c->cls_start[k + 1]);
+                if (b > a) g.maxkets[k] = std::max(g.maxkets[k], b - a);
+            }
+            for (int r = r0; r < r1; ++r)
+                g.nquartets += (long long)c->blk_nsh[I] * c->blk_nsh[J] * c->blk_nsh[c->pair_I[r]] * c->blk_nsh[c->pair_J[r]];
             // ---- J views
             for (int ra = r0; ra < r1; ra += kRunMax) {
                 const int cnt = std::min(kRunMax, r1 - ra);
                 for (int rt = 0; rt < rowtiles(nI * nJ); ++rt)
-                    items.push_back(DigestItem{0, 0, (unsigned short)rt, ra, 0, cnt});
+                    jitems.push_back(DigestItem{0, 0, (unsigned short)rt, ra, 0, cnt, sub});
             }
             for (int r = r0; r < r1; ++r) {
                 const int nK = c->blk_nao[c->pair_I[r]], nL = c->blk_nao[c->pair_J[r]];
                 for (int rt = 0; rt < rowtiles(nK * nL); ++rt)
-                    items.push_back(DigestItem{1, 0, (unsigned short)rt, r, 0, 1});
+                    jitems.push_back(DigestItem{1, 0, (unsigned short)rt, r, 0, 1, sub});
             }
-            ch.nitemsJ = (int)((long long)items.size() - ch.item0);
-            const size_t k_first = items.size();
             // ---- K views 2,3: runs of consecutive ranks with the same K (L consecutive by construction)
             for (int ra = r0; ra < r1;) {
                 const int K = c->pair_I[ra];
@@ -95,8 +145,8 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
                     const int rows = (view == 2 ? nI : nJ) * nK;
                     for (int partner = 0; partner < 2; ++partner)
                         for (int rt = 0; rt < rowtiles(rows); ++rt)
-                            items.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned short)rt, K,
-                                                       c->pair_J[ra], rb - ra});
+                            kitems.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned short)rt, K,
+                                                        c->pair_J[ra], rb - ra, sub});
                 }
                 ra = rb;
             }
@@ -114,23 +164,17 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
                         const int rows = (view == 4 ? nI : nJ) * nL;
                         for (int partner = 0; partner < 2; ++partner)
                             for (int rt = 0; rt < rowtiles(rows); ++rt)
-                                items.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned short)rt, L,
-                                                           ks[a], (int)(b - a)});
+                                kitems.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned short)rt, L,
+                                                            ks[a], (int)(b - a), sub});
                     }
                     a = b;
                 }
                 ks.clear();
             }
-            ch.nitemsK = (int)((long long)items.size() - ch.item0) - ch.nitemsJ;
-            // longest runs first: shortens the tail of each launch
-            auto longer = [](const DigestItem& a, const DigestItem& b) { return a.count > b.count; };
-            std::stable_sort(items.begin() + ch.item0, items.begin() + k_first, longer);
-            std::stable_sort(items.begin() + k_first, items.end(), longer);
-            ch.buf = (int)(c->chunks.size() & 1);
-            c->chunks.push_back(ch);
             r0 = r1;
         }
     }
+    close_group();
 }
 
 }  // namespace ltjk

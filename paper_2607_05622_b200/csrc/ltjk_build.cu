@@ -123,7 +123,7 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     // ---- panel staging ring: L2-sized by default, never below one panel
     size_t freeb = 0, totb = 0;
     LTJK_CUDA(c, cudaMemGetInfo(&freeb, &totb));
-    long long bytes = c->scratch_bytes > 0 ? c->scratch_bytes : (96ll << 20);
+    long long bytes = c->scratch_bytes > 0 ? c->scratch_bytes : (512ll << 20);
     bytes = std::min<long long>(bytes, (long long)(0.6 * (double)freeb));
     long long total = c->koff[npair] * c->koff[npair];      // never need more than everything at once
     c->panel_half = std::max<long long>(std::min<long long>(bytes / 16, total), maxpanel);
@@ -133,7 +133,7 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     std::vector<DigestItem> items;
     build_work(c, items);
     c->n_items = (long long)items.size();
-    if ((rc = upload(c, &c->d_items, items)) || (rc = upload(c, &t.sh_ao, c->sh_ao_int)) ||
+    if ((rc = upload(c, &c->d_items, items)) || (rc = upload(c, &c->d_subs, c->subs)) || (rc = upload(c, &t.sh_ao, c->sh_ao_int)) ||
         (rc = upload(c, &t.blk_sh0, c->blk_sh0)) || (rc = upload(c, &t.blk_nsh, c->blk_nsh)) ||
         (rc = upload(c, &t.blk_ao0, c->blk_ao0)) || (rc = upload(c, &t.blk_nao, c->blk_nao)) ||
         (rc = upload(c, &t.pair_I, c->pair_I)) || (rc = upload(c, &t.pair_J, c->pair_J)) ||
@@ -178,42 +178,29 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
     cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
     if (c->timing) { cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventCreate(&e2); }
 
-    // class segments of the rank order
-    int cls_start[7];
-    {
-        int r = 0;
-        for (int cls = 0; cls < 6; ++cls) {
-            cls_start[cls] = r;
-            while (r < (int)c->pair_I.size() && pair_class(c->blk_l[c->pair_I[r]], c->blk_l[c->pair_J[r]]) == cls) ++r;
-        }
-        cls_start[6] = r;
-    }
-    // Two-stream pipeline over the two halves of the panel ring: ERI(c+1) on eri_stream overlaps digest(c) on
-    // the context stream (both are DFMA-bound; the overlap fills the tail of each launch).  Timing mode serialises
-    // the two phases on the context stream so that per-phase durations are those of the kernels alone.
+    // Two-stream pipeline over the two halves of the panel ring: ERI(g+1) on eri_stream overlaps digest(g) on
+    // the context stream (both are DFMA-bound; the overlap fills launch tails and hides the long single-thread
+    // latency of the high-l quartet classes).  Timing mode serialises the two phases on the context stream so
+    // that per-phase durations are those of the kernels alone.
     c->eri_stream = c->timing ? c->stream : c->own_stream;
     if (!c->timing) {
         LTJK_CUDA(c, cudaEventRecord(c->ev_start, c->stream));          // everything enqueued before this build
         LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_start, 0));
     }
-    long long ci = 0;
-    for (const Chunk& ch : c->chunks) {
-        const int cb = pair_class(c->blk_l[ch.I], c->blk_l[ch.J]);
-        if (!c->timing && ci >= 2) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[ch.buf], 0));
+    long long gi = 0;
+    for (const Group& gr : c->groups) {
+        if (!c->timing && gi >= 2) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[gr.buf], 0));
         if (c->timing) cudaEventRecord(e0, c->stream);
-        for (int ck = 0; ck <= cb; ++ck) {
-            const int ra = std::max(ch.r0, cls_start[ck]), rb = std::min(ch.r1, cls_start[ck + 1]);
-            if (ra >= rb) continue;
-            if ((rc = launch_eri_panels(c, ch, ra, rb, cb, ck))) return rc;
-        }
+        for (int ck = 0; ck <= gr.cb; ++ck)
+            if ((rc = launch_eri_panels(c, gr, ck))) return rc;
         if (c->timing) cudaEventRecord(e1, c->stream);
         else {
-            LTJK_CUDA(c, cudaEventRecord(c->ev_eri[ch.buf], c->eri_stream));
-            LTJK_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_eri[ch.buf], 0));
+            LTJK_CUDA(c, cudaEventRecord(c->ev_eri[gr.buf], c->eri_stream));
+            LTJK_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_eri[gr.buf], 0));
         }
-        if ((rc = launch_digest(c, ch, nDp, J != nullptr, K != nullptr))) return rc;
-        if (!c->timing) LTJK_CUDA(c, cudaEventRecord(c->ev_dig[ch.buf], c->stream));
-        ++ci;
+        if ((rc = launch_digest(c, gr, nDp, J != nullptr, K != nullptr))) return rc;
+        if (!c->timing) LTJK_CUDA(c, cudaEventRecord(c->ev_dig[gr.buf], c->stream));
+        ++gi;
         if (c->timing) {
             cudaEventRecord(e2, c->stream);
             cudaEventSynchronize(e2);
@@ -221,13 +208,8 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
             cudaEventElapsedTime(&a, e0, e1); cudaEventElapsedTime(&b, e1, e2);
             c->st_eri_ms += a; c->st_digest_ms += b;
         }
-        // statistics: shell quartets evaluated and digestion flops of this chunk
-        const long long nshI = c->blk_nsh[ch.I], nshJ = c->blk_nsh[ch.J];
-        const long long nIJ = (long long)c->blk_nao[ch.I] * c->blk_nao[ch.J];
-        for (int r = ch.r0; r < ch.r1; ++r)
-            c->st_quartets += nshI * nshJ * c->blk_nsh[c->pair_I[r]] * c->blk_nsh[c->pair_J[r]];
-        const double ints = (double)nIJ * (double)(c->koff[ch.r1] - c->koff[ch.r0]);
-        c->st_digest_flops += 2.0 * ints * nDp * ((J ? 2.0 : 0.0) + (K ? 8.0 : 0.0));
+        c->st_quartets += gr.nquartets;
+        c->st_digest_flops += 2.0 * gr.nints * nDp * ((J ? 2.0 : 0.0) + (K ? 8.0 : 0.0));
     }
     if (c->timing) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2); }
     if ((rc = launch_unpack_results(c, nD, nDp, J, K))) return rc;

@@ -28,12 +28,12 @@ constexpr int kMaxNC = 1024;   // max columns of one panel view (block AO count 
 struct DigestArgs {
     DevTables t;
     const DigestItem* items;
+    const SubChunk* subs;
     const double* panel;
     const double* Dt;
     const double* Dst;
     double* Jt;
     double* Kt;
-    int I, J, r0;
     int nDp;
 };
 
@@ -71,11 +71,28 @@ __global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
     const DigestItem it = g.items[blockIdx.x];
     const int n0 = blockIdx.y * (32 * TN);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int N = T.nao, nDp = g.nDp;
     const int view = it.view;
     const bool partner = it.partner != 0;
-    const int I = g.I, J = g.J;
+    const SubChunk sc_ = g.subs[it.sub];
+    const int I = sc_.I, J = sc_.J;
+    const int N = T.nao, nDp = g.nDp;
     const int nI = T.blk_nao[I], nJ = T.blk_nao[J];
+    // Warp w owns rows 8w..8w+7 of the CTA tile and all 32 TN columns (lane + 32 t): A is a broadcast LDS.128,
+    // B a conflict-free LDS.64.  (A 4 x 8 lane tiling was measured: same speed -- multicast LDS costs the same
+    // wavefronts -- and it cannot skip the warps of a ragged last row tile, which this mapping can.)
+    const int trow = w * 8;
+    const int tcol = lane;
+    int R1, R2;                               // row blocks: constant over the run by construction
+    switch (view) {
+    case 0: R1 = I; R2 = J; break;
+    case 1: R1 = T.pair_I[it.a]; R2 = T.pair_J[it.a]; break;
+    case 2: R1 = I; R2 = it.a; break;
+    case 3: R1 = J; R2 = it.a; break;
+    case 4: R1 = I; R2 = it.a; break;
+    default: R1 = J; R2 = it.a; break;
+    }
+    const int nrows_all = T.blk_nao[R1] * T.blk_nao[R2];
+    const bool warp_active = it.rowtile * kMT + trow < nrows_all;   // ragged last tile: idle warps skip the DFMAs
 
     double acc[8][TN];
 #pragma unroll
@@ -83,7 +100,6 @@ __global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
 #pragma unroll
         for (int t = 0; t < TN; ++t) acc[r][t] = 0.0;
 
-    int R1 = 0, R2 = 0;                       // row blocks of the LAST step (constant over the run by construction)
     const double* __restrict__ Bmat = (view <= 1) ? g.Dst : g.Dt;
     const bool rowContig = (view == 1 || view >= 4);   // l (unit stride) is a row index
 
@@ -93,16 +109,16 @@ __global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
         else if (view <= 3) { K = it.a; L = it.b + s; rank = T.rank_of[K * T.nblk + L]; }
         else { L = it.a; K = it.b + s; rank = T.rank_of[K * T.nblk + L]; }
         const int nK = T.blk_nao[K], nL = T.blk_nao[L];
-        const double* __restrict__ P = g.panel + (T.koff[rank] - T.koff[g.r0]) * (long long)(nI * nJ);
+        const double* __restrict__ P = g.panel + sc_.base + (T.koff[rank] - T.koff[sc_.r0]) * (long long)(nI * nJ);
         const int sI = nJ * nK * nL, sJ = nK * nL, sK = nL, sL = 1;
         int C1, C2, sR1, sR2, sC1, sC2;
         switch (view) {
-        case 0: R1 = I; R2 = J; C1 = K; C2 = L; sR1 = sI; sR2 = sJ; sC1 = sK; sC2 = sL; break;
-        case 1: R1 = K; R2 = L; C1 = I; C2 = J; sR1 = sK; sR2 = sL; sC1 = sI; sC2 = sJ; break;
-        case 2: R1 = I; R2 = K; C1 = J; C2 = L; sR1 = sI; sR2 = sK; sC1 = sJ; sC2 = sL; break;
-        case 3: R1 = J; R2 = K; C1 = I; C2 = L; sR1 = sJ; sR2 = sK; sC1 = sI; sC2 = sL; break;
-        case 4: R1 = I; R2 = L; C1 = J; C2 = K; sR1 = sI; sR2 = sL; sC1 = sJ; sC2 = sK; break;
-        default: R1 = J; R2 = L; C1 = I; C2 = K; sR1 = sJ; sR2 = sL; sC1 = sI; sC2 = sK; break;
+        case 0: C1 = K; C2 = L; sR1 = sI; sR2 = sJ; sC1 = sK; sC2 = sL; break;
+        case 1: C1 = I; C2 = J; sR1 = sK; sR2 = sL; sC1 = sI; sC2 = sJ; break;
+        case 2: C1 = J; C2 = L; sR1 = sI; sR2 = sK; sC1 = sJ; sC2 = sL; break;
+        case 3: C1 = I; C2 = L; sR1 = sJ; sR2 = sK; sC1 = sI; sC2 = sL; break;
+        case 4: C1 = J; C2 = K; sR1 = sI; sR2 = sL; sC1 = sJ; sC2 = sK; break;
+        default: C1 = I; C2 = K; sR1 = sJ; sR2 = sL; sC1 = sI; sC2 = sK; break;
         }
         const int nR2 = T.blk_nao[R2], nrows = T.blk_nao[R1] * nR2;
         const int nC2 = T.blk_nao[C2], nC = T.blk_nao[C1] * nC2;
@@ -121,28 +137,40 @@ __global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
         __syncthreads();
 
         const int nch = (nC + kKC - 1) / kKC;
+        // Loader: everything that does not depend on the chunk is hoisted out of the chunk loop.
+        //   A tile (kKC x kMT doubles, 4 per thread): rowContig -> fixed row m, columns k = (tid>>6)+4e;
+        //                                             else      -> fixed column k, rows m = (tid>>4)+16e.
+        //   B tile: warp w copies rows k = w and w+8, lanes stride the 16-byte pieces of the row.
+        const int am = rowContig ? (tid & 63) : (tid >> 4);
+        const int ak = rowContig ? (tid >> 6) : (tid & 15);
+        int aro[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) aro[e] = S.rowoff[rowContig ? am : am + 16 * e];
         auto load = [&](int st, int ch) {
-            // A tile: kKC x kMT elements, 4 per thread
+            if (rowContig) {
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                int m, k;
-                if (rowContig) { m = tid & 63; k = (tid >> 6) + 4 * e; }
-                else { k = tid & 15; m = (tid >> 4) + 16 * e; }
-                const int cidx = ch * kKC + k;
-                const int ro = S.rowoff[m];
-                const bool ok = (ro >= 0) && (cidx < nC);
-                const double* src = ok ? (P + ro + S.acol[cidx]) : P;
-                cp_async8(&S.A[st][k][m], src, ok);
+                for (int e = 0; e < 4; ++e) {
+                    const int k = ak + 4 * e, cidx = ch * kKC + k;
+                    const bool ok = (aro[0] >= 0) && (cidx < nC);
+                    cp_async8(&S.A[st][k][am], ok ? (P + aro[0] + S.acol[cidx]) : P, ok);
+                }
+            } else {
+                const int cidx = ch * kKC + ak;
+                const bool cok = cidx < nC;
+                const int co = cok ? S.acol[cidx] : 0;
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const bool ok = cok && (aro[e] >= 0);
+                    cp_async8(&S.A[st][ak][am + 16 * e], ok ? (P + aro[e] + co) : P, ok);
+                }
             }
-            // B tile: kKC rows of 32*TN doubles, 16-byte pieces
 #pragma unroll
-            for (int e = 0; e < TN; ++e) {
-                const int id = tid + 256 * e;
-                const int k = id / (16 * TN), piece = id % (16 * TN);
-                const int cidx = ch * kKC + k;
+            for (int h = 0; h < 2; ++h) {
+                const int k = w + 8 * h, cidx = ch * kKC + k;
                 const bool ok = cidx < nC;
-                const double* src = ok ? (Bmat + (size_t)S.bcol[cidx] * nDp + n0 + piece * 2) : Bmat;
-                cp_async16(&S.B[st][k][piece * 2], src, ok);
+                const double* src = ok ? (Bmat + (size_t)S.bcol[cidx] * nDp + n0) : Bmat;
+#pragma unroll
+                for (int pc = lane; pc < 16 * TN; pc += 32) cp_async16(&S.B[st][k][pc * 2], src + (ok ? pc * 2 : 0), ok);
             }
         };
 #pragma unroll
@@ -157,18 +185,20 @@ __global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
             if (nxt < nch) load(nxt % kStages, nxt);
             cp_async_commit();
             const int st = ch % kStages;
+            if (warp_active) {
 #pragma unroll
             for (int k = 0; k < kKC; ++k) {
-                const double2* ap = reinterpret_cast<const double2*>(&S.A[st][k][w * 8]);
+                const double2* ap = reinterpret_cast<const double2*>(&S.A[st][k][trow]);
                 const double2 a01 = ap[0], a23 = ap[1], a45 = ap[2], a67 = ap[3];
                 const double a[8] = {a01.x, a01.y, a23.x, a23.y, a45.x, a45.y, a67.x, a67.y};
                 double b[TN];
 #pragma unroll
-                for (int t = 0; t < TN; ++t) b[t] = S.B[st][k][lane + 32 * t];
+                for (int t = 0; t < TN; ++t) b[t] = S.B[st][k][tcol + 32 * t];
 #pragma unroll
                 for (int r = 0; r < 8; ++r)
 #pragma unroll
                     for (int t = 0; t < TN; ++t) acc[r][t] = fma(a[r], b[t], acc[r][t]);
+            }
             }
         }
         cp_async_wait<0>();
@@ -180,11 +210,11 @@ __global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
     const int aoR1 = T.blk_ao0[R1], aoR2 = T.blk_ao0[R2];
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
-        const int m = it.rowtile * kMT + w * 8 + r;
+        const int m = it.rowtile * kMT + trow + r;
         if (m < nrows) {
             const int r1 = m / nR2, r2 = m % nR2;
             const size_t row = partner ? (size_t)(aoR2 + r2) * N + aoR1 + r1 : (size_t)(aoR1 + r1) * N + aoR2 + r2;
-            double* o = Out + row * nDp + n0 + lane;
+            double* o = Out + row * nDp + n0 + tcol;
 #pragma unroll
             for (int t = 0; t < TN; ++t) atomicAdd(o + 32 * t, acc[r][t]);
         }
@@ -218,15 +248,15 @@ void digest_colblocks(int nD, int* TN, int* ncolblk)
     *TN = best_tn; *ncolblk = best_nb;
 }
 
-int launch_digest(ltjk_ctx* c, const Chunk& ch, int nDp, bool doJ, bool doK)
+int launch_digest(ltjk_ctx* c, const Group& ch, int nDp, bool doJ, bool doK)
 {
     const long long first = ch.item0 + (doJ ? 0 : ch.nitemsJ);
     const int nitems = (doJ ? ch.nitemsJ : 0) + (doK ? ch.nitemsK : 0);
     if (nitems == 0) return LTJK_OK;
     DigestArgs g;
-    g.t = c->t; g.items = c->d_items + first; g.panel = c->d_panel + (size_t)ch.buf * c->panel_half;
+    g.t = c->t; g.items = c->d_items + first; g.subs = c->d_subs; g.panel = c->d_panel + (size_t)ch.buf * c->panel_half;
     g.Dt = c->Dt; g.Dst = c->Dst; g.Jt = c->Jt; g.Kt = c->Kt;
-    g.I = ch.I; g.J = ch.J; g.r0 = ch.r0; g.nDp = nDp;
+    g.nDp = nDp;
     int TN, nb;
     digest_colblocks(nDp, &TN, &nb);
     if (nb * TN * 32 != nDp) return set_err(c, LTJK_EINVAL, "internal: nDp is not a whole number of column blocks");

@@ -83,33 +83,35 @@ int launch_schwarz(ltjk_ctx* c, const int* lrange /* host: first internal shell 
 // a6 + a7: panels of one class segment.  Thread -> (ket rank r in [ra,rb), shell quartet inside the block quartet).
 struct EriArgs {
     DevTables t;
-    int I, J, rIJ, r0;     // chunk: bra blocks, bra rank, first ket rank of the chunk (panel base origin)
-    int ra, rb;            // ket ranks of this launch (one pair class)
+    const SubChunk* subs;  // sub-chunks of the group; blockIdx.y selects one
+    int ca, cb_;           // rank range [ca, cb_) of the launch's ket pair class
     int mJ, mK, mL;        // max shells per block of the launch's l_J, l_K, l_L (thread-index decode)
     int qn;                // mI*mJ*mK*mL
     double tau;
-    double* panel;
+    double* panel;         // ring half
 };
 
 template <int LA, int LB, int LC, int LD>
 // (64,4): without a min-blocks hint ptxas drops the heavy classes to 32 registers and spills ~80 KB per thread
 __global__ void __launch_bounds__(64, 4) eri_panel_kernel(const EriArgs g)
 {
+    const SubChunk sc_ = g.subs[blockIdx.y];
+    const int ra = max(sc_.r0, g.ca), rb = min(sc_.r1, g.cb_);
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int r = g.ra + (int)(t / g.qn);
-    if (r >= g.rb) return;
+    const int r = ra + (int)(t / g.qn);
+    if (r >= rb) return;
     int q = (int)(t % g.qn);
     const int sd = q % g.mL; q /= g.mL;
     const int sc = q % g.mK; q /= g.mK;
     const int sb = q % g.mJ;
     const int sa = q / g.mJ;
     const DevTables& T = g.t;
-    const int I = g.I, J = g.J, K = T.pair_I[r], L = T.pair_J[r];
+    const int I = sc_.I, J = sc_.J, K = T.pair_I[r], L = T.pair_J[r];
     if (sa >= T.blk_nsh[I] || sb >= T.blk_nsh[J] || sc >= T.blk_nsh[K] || sd >= T.blk_nsh[L]) return;
     const int A = T.blk_sh0[I] + sa, B = T.blk_sh0[J] + sb, C = T.blk_sh0[K] + sc, D = T.blk_sh0[L] + sd;
     constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
     const int nJ = T.blk_nao[J], nK = T.blk_nao[K], nL = T.blk_nao[L];
-    const long long base = (T.koff[r] - T.koff[g.r0]) * (long long)(T.blk_nao[I] * nJ);
+    const long long base = sc_.base + (T.koff[r] - T.koff[sc_.r0]) * (long long)(T.blk_nao[I] * nJ);
     double* __restrict__ P = g.panel + base + ((long long)(sa * NA) * nJ + sb * NB) * (nK * nL) + (sc * NC) * nL + sd * ND;
     const int sI = nJ * nK * nL, sJ = nK * nL, sK = nL;
 
@@ -125,7 +127,7 @@ __global__ void __launch_bounds__(64, 4) eri_panel_kernel(const EriArgs g)
     double scale = 1.0;
     if (I == J) scale *= 0.5;
     if (K == L) scale *= 0.5;
-    if (r == g.rIJ) scale *= 0.5;
+    if (r == sc_.rIJ) scale *= 0.5;
     double out[NA * NB * NC * ND];
     eri_quartet<LA, LB, LC, LD>(T.pair_rec + ((size_t)A * T.nshell + B) * T.rec_stride,
                                 T.pair_rec + ((size_t)C * T.nshell + D) * T.rec_stride, T.boys, out);
@@ -140,13 +142,14 @@ __global__ void __launch_bounds__(64, 4) eri_panel_kernel(const EriArgs g)
 static const int kClsLa[6] = {0, 1, 1, 2, 2, 2}, kClsLb[6] = {0, 0, 1, 0, 1, 2};
 
 template <int CB, int CK>
-static int launch_cls(ltjk_ctx* c, const EriArgs& g)
+static int launch_cls(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
 {
     constexpr int la[6] = {0, 1, 1, 2, 2, 2}, lb[6] = {0, 0, 1, 0, 1, 2};
     if constexpr (CK <= CB) {
-        const long long nthr = (long long)(g.rb - g.ra) * g.qn;
+        const long long nthr = (long long)maxkets * g.qn;
         const int bs = 64;
-        eri_panel_kernel<la[CB], lb[CB], la[CK], lb[CK]><<<(unsigned)((nthr + bs - 1) / bs), bs, 0, c->eri_stream>>>(g);
+        eri_panel_kernel<la[CB], lb[CB], la[CK], lb[CK]>
+            <<<dim3((unsigned)((nthr + bs - 1) / bs), nsub), bs, 0, c->eri_stream>>>(g);
         LTJK_CUDA(c, cudaGetLastError());
         return LTJK_OK;
     } else {
@@ -155,36 +158,40 @@ static int launch_cls(ltjk_ctx* c, const EriArgs& g)
 }
 
 template <int CB>
-static int launch_cls_k(ltjk_ctx* c, int ck, const EriArgs& g)
+static int launch_cls_k(ltjk_ctx* c, int ck, const EriArgs& g, int mk, int ns)
 {
     switch (ck) {
-    case 0: return launch_cls<CB, 0>(c, g);
-    case 1: return launch_cls<CB, 1>(c, g);
-    case 2: return launch_cls<CB, 2>(c, g);
-    case 3: return launch_cls<CB, 3>(c, g);
-    case 4: return launch_cls<CB, 4>(c, g);
-    default: return launch_cls<CB, 5>(c, g);
+    case 0: return launch_cls<CB, 0>(c, g, mk, ns);
+    case 1: return launch_cls<CB, 1>(c, g, mk, ns);
+    case 2: return launch_cls<CB, 2>(c, g, mk, ns);
+    case 3: return launch_cls<CB, 3>(c, g, mk, ns);
+    case 4: return launch_cls<CB, 4>(c, g, mk, ns);
+    default: return launch_cls<CB, 5>(c, g, mk, ns);
     }
 }
 
-int launch_eri_panels(ltjk_ctx* c, const Chunk& ch, int ra, int rb, int cb, int ck)
+int launch_eri_panels(ltjk_ctx* c, const Group& gr, int ck)
 {
+    if (gr.maxkets[ck] == 0) return LTJK_OK;
+    const int cb = gr.cb;
     EriArgs g;
     g.t = c->t;
-    g.I = ch.I; g.J = ch.J; g.rIJ = ch.rIJ; g.r0 = ch.r0; g.ra = ra; g.rb = rb;
+    g.subs = c->d_subs + gr.sub0;
+    g.ca = c->cls_start[ck]; g.cb_ = c->cls_start[ck + 1];
     const int mI = c->max_nsh_l[kClsLa[cb]];
     g.mJ = c->max_nsh_l[kClsLb[cb]]; g.mK = c->max_nsh_l[kClsLa[ck]]; g.mL = c->max_nsh_l[kClsLb[ck]];
     g.qn = mI * g.mJ * g.mK * g.mL;
     g.tau = c->tau;
-    g.panel = c->d_panel + (size_t)ch.buf * c->panel_half;
+    g.panel = c->d_panel + (size_t)gr.buf * c->panel_half;
     c->st_launches++;
+    const int mk = gr.maxkets[ck], ns = gr.nsub;
     switch (cb) {
-    case 0: return launch_cls_k<0>(c, ck, g);
-    case 1: return launch_cls_k<1>(c, ck, g);
-    case 2: return launch_cls_k<2>(c, ck, g);
-    case 3: return launch_cls_k<3>(c, ck, g);
-    case 4: return launch_cls_k<4>(c, ck, g);
-    default: return launch_cls_k<5>(c, ck, g);
+    case 0: return launch_cls_k<0>(c, ck, g, mk, ns);
+    case 1: return launch_cls_k<1>(c, ck, g, mk, ns);
+    case 2: return launch_cls_k<2>(c, ck, g, mk, ns);
+    case 3: return launch_cls_k<3>(c, ck, g, mk, ns);
+    case 4: return launch_cls_k<4>(c, ck, g, mk, ns);
+    default: return launch_cls_k<5>(c, ck, g, mk, ns);
     }
 }
 

@@ -30,7 +30,16 @@ struct DevTables {
     int* ao_perm = nullptr;        // [nao]      internal AO -> caller AO
 };
 
-// One digestion work item (16 bytes): a row tile of one output block accumulated over a run of panels.
+// A sub-chunk: the panels (IJ|KL) of one bra block pair and a run of ket ranks [r0,r1), contiguous in one half of
+// the panel ring starting at `base`.
+struct SubChunk {
+    int I, J, rIJ;          // bra block pair and its rank
+    int r0, r1;             // ket ranks [r0, r1)
+    int pad;
+    long long base;         // offset (doubles) of the first panel inside the ring half
+};
+
+// One digestion work item (20 bytes): a row tile of one output block accumulated over a run of panels.
 struct DigestItem {
     unsigned char view;     // 0 JIJ, 1 JKL, 2 KIK, 3 KJK, 4 KIL, 5 KJL
     unsigned char partner;  // K views: 0 -> K[(r1,r2)] with D[(c1,c2)];  1 -> K[(r2,r1)] with D[(c2,c1)]
@@ -38,14 +47,20 @@ struct DigestItem {
     int a;                  // JIJ/JKL: first ket rank;  KIK/KJK: K;  KIL/KJL: L
     int b;                  // KIK/KJK: first L;  KIL/KJL: first K
     int count;              // panels in the run
+    int sub;                // sub-chunk (global index)
 };
 
-struct Chunk {
-    int I, J, rIJ;          // bra block pair and its rank
-    int r0, r1;             // ket ranks [r0, r1)
+// A group: consecutive sub-chunks of one bra class that fit one ring half; one ERI launch per ket class and one
+// digestion launch per group.
+struct Group {
+    int sub0, nsub;         // sub-chunks [sub0, sub0+nsub)
+    int cb;                 // bra pair class
+    int buf;                // ring half
     long long item0;        // first digest item: nitemsJ J-view items, then nitemsK K-view items
     int nitemsJ, nitemsK;
-    int buf;                // which half of the panel ring (chunks alternate)
+    int maxkets[6];         // per ket class: max number of kets of that class in one sub-chunk
+    long long nquartets;    // shell quartets evaluated
+    double nints;           // integrals in the panels
 };
 
 }  // namespace ltjk
@@ -70,13 +85,16 @@ struct ltjk_ctx {
     std::vector<int> pair_I, pair_J, rank_of;
     std::vector<long long> koff;
     std::vector<double> Qhost;            // internal order [nshell*nshell]
-    std::vector<ltjk::Chunk> chunks;
+    std::vector<ltjk::SubChunk> subs;
+    std::vector<ltjk::Group> groups;
+    int cls_start[7] = {0, 0, 0, 0, 0, 0, 0};   // first rank of each pair class
     int max_nsh_l[3] = {0, 0, 0};         // max shells per block for each l
     double tau = 0.0;
     long long n_quartets_kept = 0;
 
     ltjk::DevTables t;
     ltjk::DigestItem* d_items = nullptr;
+    ltjk::SubChunk* d_subs = nullptr;
     long long n_items = 0;
     double* d_panel = nullptr;            // integral panel staging ring (L2-sized)
     long long panel_cap = 0;              // doubles (both halves)
@@ -118,12 +136,12 @@ void digest_colblocks(int nD, int* TN, int* ncolblk);
 int launch_pair_records(ltjk_ctx* c, const double* d_xyz, const int* d_atom, const int* d_l, const int* d_nprim,
                         const int* d_poff, const double* d_exps, const double* d_coef, const int* d_int2ext);
 int launch_schwarz(ltjk_ctx* c, const int* lrange_host);
-int launch_eri_panels(ltjk_ctx* c, const Chunk& ch, int ra, int rb, int cb, int ck);
+int launch_eri_panels(ltjk_ctx* c, const Group& g, int ck);
 int launch_eri_single(ltjk_ctx* c, int A, int B, int C, int D, int la, int lb, int lc, int ld, double* d_out);
 int launch_boys_debug(ltjk_ctx* c, int mmax, int n, const double* d_T, double* d_F);
 
 // ltjk_digest.cu
-int launch_digest(ltjk_ctx* c, const Chunk& ch, int nDp, bool doJ, bool doK);
+int launch_digest(ltjk_ctx* c, const Group& g, int nDp, bool doJ, bool doK);
 int launch_pack_densities(ltjk_ctx* c, int nD, int nDp, const double* D);
 int launch_unpack_results(ltjk_ctx* c, int nD, int nDp, double* J, double* K);
 int bench_dfma(ltjk_ctx* c, double* tflops);
