@@ -43,8 +43,9 @@ int ltjk_create(ltjk_ctx** out, int device, void* cuda_stream);
 int ltjk_destroy(ltjk_ctx* ctx);
 const char* ltjk_last_error(const ltjk_ctx* ctx);
 
-/* Upper bound, in bytes, on the integral-panel scratch the context may allocate (default 32 GiB, clamped to
- * 60 % of free device memory at build_shell_pairs time).  Must be called before ltjk_build_shell_pairs. */
+/* Upper bound, in bytes, on the integral-panel staging ring the context allocates (two halves; default 8 GiB or a
+ * quarter of the free device memory, whichever is smaller; always clamped to 60 % of free memory and never below two
+ * panels).  Must be called before ltjk_build_shell_pairs. */
 int ltjk_set_scratch_bytes(ltjk_ctx* ctx, long long bytes);
 
 /* Basis upload (step a1).  HOST pointers, copied.

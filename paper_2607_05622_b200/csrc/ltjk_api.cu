@@ -128,30 +128,46 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
             for (int ra = r0; ra < r1; ra += kRunMax) {
                 const int cnt = std::min(kRunMax, r1 - ra);
                 for (int rt = 0; rt < rowtiles(nI * nJ); ++rt)
-                    jitems.push_back(DigestItem{0, 0, (unsigned short)rt, ra, 0, cnt, sub});
+                    jitems.push_back(DigestItem{0, 0, (unsigned char)rt, 1, ra, 0, cnt, sub});
             }
             for (int r = r0; r < r1; ++r) {
                 const int nK = c->blk_nao[c->pair_I[r]], nL = c->blk_nao[c->pair_J[r]];
                 for (int rt = 0; rt < rowtiles(nK * nL); ++rt)
-                    jitems.push_back(DigestItem{1, 0, (unsigned short)rt, r, 0, 1, sub});
+                    jitems.push_back(DigestItem{1, 0, (unsigned char)rt, 1, r, 0, 1, sub});
             }
-            // ---- K views 2,3: runs of consecutive ranks with the same K (L consecutive by construction)
+            // ---- K views.  Diagonal block quartets: the panel is symmetric under i<->j when I == J and under
+            // k<->l when K == L, which makes pairs of K images identical; they are digested once with weight 2:
+            //   I == J : KJK == KIK and KJL == KIL   -> views 3, 5 dropped, views 2, 4 doubled
+            //   K == L : KIL == KIK and KJL == KJK   -> views 4, 5 dropped, views 2, 3 doubled
+            const bool dI = (I == J);
+            auto push_k = [&](int view, int mult, int fixed, int first, int cnt, int rows) {
+                for (int partner = 0; partner < 2; ++partner)
+                    for (int rt = 0; rt < rowtiles(rows); ++rt)
+                        kitems.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned char)rt,
+                                                    (unsigned char)mult, fixed, first, cnt, sub});
+            };
+            // views 2,3: runs of consecutive ranks with the same K (L consecutive by construction); a K == L
+            // panel ends the run it would belong to and is digested on its own with the extra weight
             for (int ra = r0; ra < r1;) {
                 const int K = c->pair_I[ra];
-                int rb = ra + 1;
-                while (rb < r1 && c->pair_I[rb] == K && c->pair_J[rb] == c->pair_J[rb - 1] + 1 && rb - ra < kRunMax) ++rb;
                 const int nK = c->blk_nao[K];
-                for (int view = 2; view <= 3; ++view) {
-                    const int rows = (view == 2 ? nI : nJ) * nK;
-                    for (int partner = 0; partner < 2; ++partner)
-                        for (int rt = 0; rt < rowtiles(rows); ++rt)
-                            kitems.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned short)rt, K,
-                                                        c->pair_J[ra], rb - ra, sub});
+                if (c->pair_J[ra] == K) {                                   // K == L
+                    push_k(2, dI ? 4 : 2, K, K, 1, nI * nK);
+                    if (!dI) push_k(3, 2, K, K, 1, nJ * nK);
+                    ++ra;
+                    continue;
                 }
+                int rb = ra + 1;
+                while (rb < r1 && c->pair_I[rb] == K && c->pair_J[rb] == c->pair_J[rb - 1] + 1 && c->pair_J[rb] != K &&
+                       rb - ra < kRunMax)
+                    ++rb;
+                push_k(2, dI ? 2 : 1, K, c->pair_J[ra], rb - ra, nI * nK);
+                if (!dI) push_k(3, 1, K, c->pair_J[ra], rb - ra, nJ * nK);
                 ra = rb;
             }
-            // ---- K views 4,5: for each L, runs of consecutive K
-            for (int r = r0; r < r1; ++r) byL[c->pair_J[r]].push_back(c->pair_I[r]);
+            // views 4,5: for each L, runs of consecutive K (K == L panels are covered by views 2,3)
+            for (int r = r0; r < r1; ++r)
+                if (c->pair_I[r] != c->pair_J[r]) byL[c->pair_J[r]].push_back(c->pair_I[r]);
             for (int L = 0; L < nblk; ++L) {
                 std::vector<int>& ks = byL[L];
                 if (ks.empty()) continue;
@@ -160,13 +176,8 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
                 for (size_t a = 0; a < ks.size();) {
                     size_t b = a + 1;
                     while (b < ks.size() && ks[b] == ks[b - 1] + 1 && (int)(b - a) < kRunMax) ++b;
-                    for (int view = 4; view <= 5; ++view) {
-                        const int rows = (view == 4 ? nI : nJ) * nL;
-                        for (int partner = 0; partner < 2; ++partner)
-                            for (int rt = 0; rt < rowtiles(rows); ++rt)
-                                kitems.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned short)rt, L,
-                                                            ks[a], (int)(b - a), sub});
-                    }
+                    push_k(4, dI ? 2 : 1, L, ks[a], (int)(b - a), nI * nL);
+                    if (!dI) push_k(5, 1, L, ks[a], (int)(b - a), nJ * nL);
                     a = b;
                 }
                 ks.clear();

@@ -123,7 +123,9 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     // ---- panel staging ring: L2-sized by default, never below one panel
     size_t freeb = 0, totb = 0;
     LTJK_CUDA(c, cudaMemGetInfo(&freeb, &totb));
-    long long bytes = c->scratch_bytes > 0 ? c->scratch_bytes : (512ll << 20);
+    // Default 8 GiB (two 4 GiB halves), at most a quarter of the free memory: measured on B200, launches that fill
+    // the GPU matter far more than keeping the panels L2-resident.
+    long long bytes = c->scratch_bytes > 0 ? c->scratch_bytes : std::min<long long>(8ll << 30, (long long)(0.25 * (double)freeb));
     bytes = std::min<long long>(bytes, (long long)(0.6 * (double)freeb));
     long long total = c->koff[npair] * c->koff[npair];      // never need more than everything at once
     c->panel_half = std::max<long long>(std::min<long long>(bytes / 16, total), maxpanel);
@@ -209,7 +211,7 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
             c->st_eri_ms += a; c->st_digest_ms += b;
         }
         c->st_quartets += gr.nquartets;
-        c->st_digest_flops += 2.0 * gr.nints * nDp * ((J ? 2.0 : 0.0) + (K ? 8.0 : 0.0));
+        c->st_digest_flops += 2.0 * gr.nints * nDp * ((J ? 2.0 : 0.0) + (K ? 8.0 : 0.0));   // images applied (folded ones included)
     }
     if (c->timing) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2); }
     if ((rc = launch_unpack_results(c, nD, nDp, J, K))) return rc;

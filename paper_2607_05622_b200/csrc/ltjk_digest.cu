@@ -205,6 +205,7 @@ __global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
     }
 
     // flush: coalesced fp64 reductions into the density-fastest accumulators
+    const double mult = (double)it.mult;
     double* __restrict__ Out = (view <= 1) ? g.Jt : g.Kt;
     const int nR2 = T.blk_nao[R2], nrows = T.blk_nao[R1] * nR2;
     const int aoR1 = T.blk_ao0[R1], aoR2 = T.blk_ao0[R2];
@@ -216,7 +217,7 @@ __global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
             const size_t row = partner ? (size_t)(aoR2 + r2) * N + aoR1 + r1 : (size_t)(aoR1 + r1) * N + aoR2 + r2;
             double* o = Out + row * nDp + n0 + tcol;
 #pragma unroll
-            for (int t = 0; t < TN; ++t) atomicAdd(o + 32 * t, acc[r][t]);
+            for (int t = 0; t < TN; ++t) atomicAdd(o + 32 * t, mult * acc[r][t]);
         }
     }
 }

@@ -43,7 +43,8 @@ struct SubChunk {
 struct DigestItem {
     unsigned char view;     // 0 JIJ, 1 JKL, 2 KIK, 3 KJK, 4 KIL, 5 KJL
     unsigned char partner;  // K views: 0 -> K[(r1,r2)] with D[(c1,c2)];  1 -> K[(r2,r1)] with D[(c2,c1)]
-    unsigned short rowtile;
+    unsigned char rowtile;
+    unsigned char mult;     // 1, 2 or 4: diagonal block quartets fold identical K images into one (see build_work)
     int a;                  // JIJ/JKL: first ket rank;  KIK/KJK: K;  KIL/KJL: L
     int b;                  // KIK/KJK: first L;  KIL/KJL: first K
     int count;              // panels in the run
