@@ -138,12 +138,12 @@ class VRR:
         eidx = range_index(la, la + lb)
         fidx = range_index(lc, lc + ld)
         nf = len(fidx)
-        outs = []
+        # every target is accumulated right after it is computed (short live ranges: fewer registers held)
         for e, ie in eidx.items():
             for f, jf in fidx.items():
                 v = self.node(e, f, 0)
-                outs.append("acc[%d] += %s;" % (ie * nf + jf, v))
-        return self.lines + outs, len(eidx), nf
+                self.lines.append("acc[%d] += %s;" % (ie * nf + jf, v))
+        return self.lines, len(eidx), nf
 
 
 def gen_hrr(la, lb):

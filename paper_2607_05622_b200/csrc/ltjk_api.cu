@@ -275,10 +275,37 @@ int ltjk_set_basis(ltjk_ctx* c, int natom, const double* xyz, int nshell, const 
     std::vector<int> ao_ext(nshell + 1, 0);
     for (int s = 0; s < nshell; ++s) ao_ext[s + 1] = ao_ext[s] + ncart(l[s]);
     c->nao = ao_ext[nshell];
-    // internal shell order: by l, then caller order
+    // internal shell order: by l, then by exponent tier (most diffuse primitive, half-octave buckets), then along a
+    // Morton curve through the centres.  Blocks cut from this order are compact in space and homogeneous in extent,
+    // so that whole block pairs fall below the Schwarz threshold and never enter the work lists (a2/a5).
     c->sh_int2ext.resize(nshell);
     for (int s = 0; s < nshell; ++s) c->sh_int2ext[s] = s;
-    std::stable_sort(c->sh_int2ext.begin(), c->sh_int2ext.end(), [&](int a, int b) { return l[a] < l[b]; });
+    {
+        double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+        for (int a = 0; a < natom; ++a)
+            for (int k = 0; k < 3; ++k) { lo[k] = std::min(lo[k], xyz[3 * a + k]); hi[k] = std::max(hi[k], xyz[3 * a + k]); }
+        const double ext = std::max({hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2], 1e-9});
+        std::vector<unsigned long long> morton(natom);
+        for (int a = 0; a < natom; ++a) {
+            unsigned long long m = 0;
+            unsigned q[3];
+            for (int k = 0; k < 3; ++k) q[k] = (unsigned)std::min(1023.0, 1023.0 * (xyz[3 * a + k] - lo[k]) / ext);
+            for (int bit = 9; bit >= 0; --bit)
+                for (int k = 0; k < 3; ++k) m = (m << 1) | ((q[k] >> bit) & 1u);
+            morton[a] = m;
+        }
+        std::vector<int> tier(nshell);
+        for (int s = 0; s < nshell; ++s) {
+            double amin = 1e300;
+            for (int p = 0; p < nprim[s]; ++p) amin = std::min(amin, exps[prim_off[s] + p]);
+            tier[s] = (int)std::floor(2.0 * std::log2(amin) + 0.5);
+        }
+        std::stable_sort(c->sh_int2ext.begin(), c->sh_int2ext.end(), [&](int a, int b) {
+            if (l[a] != l[b]) return l[a] < l[b];
+            if (tier[a] != tier[b]) return tier[a] < tier[b];
+            return morton[atom[a]] < morton[atom[b]];
+        });
+    }
     c->sh_ao_int.assign(nshell, 0);
     c->ao_perm.assign(c->nao, 0);
     int ao = 0;

@@ -103,10 +103,22 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     const int nblk = t.nblk;
     c->pair_I.clear(); c->pair_J.clear();
     c->rank_of.assign((size_t)nblk * nblk, -1);
+    // a block pair whose every shell pair has Q_AB * max(Q) < tau can never pass the quartet test: dropped here
+    std::vector<double> qblk((size_t)nblk * nblk, 0.0);
+    double qmax = 0.0;
+    for (int I = 0; I < nblk; ++I)
+        for (int J = 0; J <= I; ++J) {
+            double m = 0.0;
+            for (int a = 0; a < c->blk_nsh[I]; ++a)
+                for (int b = 0; b < c->blk_nsh[J]; ++b)
+                    m = std::max(m, c->Qhost[(size_t)(c->blk_sh0[I] + a) * ns + c->blk_sh0[J] + b]);
+            qblk[(size_t)I * nblk + J] = m;
+            qmax = std::max(qmax, m);
+        }
     for (int cls = 0; cls < 6; ++cls)
         for (int I = 0; I < nblk; ++I)
             for (int J = 0; J <= I; ++J)
-                if (pair_class(c->blk_l[I], c->blk_l[J]) == cls) {
+                if (pair_class(c->blk_l[I], c->blk_l[J]) == cls && qblk[(size_t)I * nblk + J] * qmax >= schwarz_tau) {
                     c->rank_of[(size_t)I * nblk + J] = (int)c->pair_I.size();
                     c->pair_I.push_back(I); c->pair_J.push_back(J);
                 }
