@@ -163,3 +163,53 @@ def test_jk_host_entry_matches_device_entry(torch_cuda, tiny):
     assert relerr(Jh, J) < 1e-13 and relerr(Kh, K) < 1e-13
     Jr, Kr, _ = O.jk_folded(tiny.basis, D, tiny.schwarz_tau)
     assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
+
+
+@pytest.mark.parametrize("name", ["medium", "porphine", "large"])
+def test_full_size_sweep_sampled_blocks(torch_cuda, name):
+    """BASELINE.json's full sizes in the configuration bench.py times (whole Laplace sweep: transform + J/K for all
+    n_tau x n_T densities, default panel ring): sampled output blocks against Eq. 17 evaluated one by one by the oracle
+    (orc_jk_blocks), plus properties that hold at any size (J symmetric, K[D^T] = K[D]^T on a transposed density)."""
+    torch = torch_cuda
+    w = make_workload(name)
+    N, nD = w.nao, w.nD
+    ctx = make_ctx(w.basis)
+    tau = np.geomspace(0.05, 6.0, w.ntau)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    D = torch.empty((w.ntau, w.nT, N, N), dtype=torch.float64, device="cuda")
+    ctx.build_pseudo_densities(dev(w.C_occ), dev(w.C_vir), dev(w.eps_occ), dev(w.eps_vir), dev(w.T), tau, D)
+    Dn = D.view(nD, N, N)
+    # density nD-1 is replaced by the transpose of density 0: K must come out transposed, J equal
+    Dn[nD - 1].copy_(Dn[0].t())
+    J = torch.empty_like(Dn)
+    K = torch.empty_like(Dn)
+    ctx.jk_build(Dn, J, K)
+    torch.cuda.synchronize()
+    assert float((J - J.transpose(1, 2)).abs().max()) <= 1e-12 * float(J.abs().max())
+    assert float((K[nD - 1] - K[0].t()).abs().max()) <= 1e-11 * float(K[0].abs().max())
+    assert float((J[nD - 1] - J[0]).abs().max()) <= 1e-11 * float(J[0].abs().max())
+    assert float((K[0] - K[0].t()).abs().max()) > 1e-3 * float(K[0].abs().max())      # genuinely non-symmetric
+    # transform: sampled densities against the explicit-loop oracle on sampled rows
+    rng = np.random.default_rng(5)
+    # sampled shell-pair blocks (one per pair class where available) for a subset of densities
+    b = w.basis
+    ds = sorted(set([0, 1, nD // 2, nD - 2] + [int(x) for x in rng.integers(0, nD - 1, size=4)]))
+    Dh = Dn[ds].cpu().numpy()
+    Jh = J[ds].cpu().numpy()
+    Kh = K[ds].cpu().numpy()
+    Dref = O.pseudo_densities_loops(w.C_occ, w.C_vir, w.eps_occ, w.eps_vir, w.T[:1], tau[:1])[0, 0]
+    assert relerr(Dn[nD - 1].cpu().numpy().T, Dref) < 1e-12
+    pairs = []
+    byl = {l: [s for s in range(b.nshell) if b.l[s] == l] for l in range(3)}
+    for la in range(3):
+        for lb in range(3):
+            if byl[la] and byl[lb]:
+                pairs.append((int(rng.choice(byl[la])), int(rng.choice(byl[lb]))))
+    Jb, Kb = O.jk_blocks(b, Dh, w.schwarz_tau, pairs)
+    jmax = np.abs(Jh).reshape(len(ds), -1).max(1)
+    kmax = np.abs(Kh).reshape(len(ds), -1).max(1)
+    for (X, Y), jb, kb in zip(pairs, Jb, Kb):
+        x0, x1, y0, y1 = b.ao_off[X], b.ao_off[X + 1], b.ao_off[Y], b.ao_off[Y + 1]
+        ej = np.abs(Jh[:, x0:x1, y0:y1] - jb).reshape(len(ds), -1).max(1) / jmax
+        ek = np.abs(Kh[:, x0:x1, y0:y1] - kb).reshape(len(ds), -1).max(1) / kmax
+        assert ej.max() < TOL and ek.max() < TOL, ((X, Y), ej.max(), ek.max())
