@@ -62,7 +62,7 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
     c->subs.clear();
     c->groups.clear();
     items.clear();
-    auto rowtiles = [](int rows) { return (rows + 63) / 64; };
+    auto rowtiles = [](int rows) { return (rows + kDigestRows - 1) / kDigestRows; };
     auto cls_of = [&](int r) { return pair_class(c->blk_l[c->pair_I[r]], c->blk_l[c->pair_J[r]]); };
     {
         int r = 0;

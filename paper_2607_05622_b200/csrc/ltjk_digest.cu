@@ -19,10 +19,11 @@
 
 namespace ltjk {
 
-constexpr int kMT = 64;        // rows per CTA
-constexpr int kMTP = 66;       // padded row stride of the A tile in shared memory
-constexpr int kKC = 16;        // contraction chunk
-constexpr int kStages = 3;
+constexpr int kMT = kDigestRows;   // rows per CTA (128)
+constexpr int kMTP = kMT + 2;      // padded row stride of the A tile in shared memory
+constexpr int kKC = 16;            // contraction chunk
+constexpr int kStages = 5;
+constexpr int kTM = 16;            // rows per consumer thread
 constexpr int kMaxNC = 1024;   // max columns of one panel view (block AO count squared)
 
 struct DigestArgs {
@@ -53,17 +54,56 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
+// ---- mbarrier helpers (producer/consumer pipeline inside one CTA) -------------------------------------------------
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar)
+{
+    asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+// arrive on `bar` once all cp.async issued so far by this thread have landed (the count was provisioned at init)
+__device__ __forceinline__ void mbar_arrive_on_cp_async(unsigned long long* bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(a),
+        "r"(parity)
+        : "memory");
+}
+
 template <int TN>
 struct DigestSmem {
     double A[kStages][kKC][kMTP];
     double B[kStages][kKC][32 * TN];
+    unsigned long long full[kStages];    // producer -> consumers: the stage's tiles have landed
+    unsigned long long empty[kStages];   // consumers -> producer: the stage may be refilled
     int rowoff[kMT];
     int acol[kMaxNC];
     unsigned bcol[kMaxNC];
 };
 
+constexpr int kConsumerWarps = 8;
+constexpr int kProducerWarps = 4;
+constexpr int kProducerThreads = kProducerWarps * 32;
+constexpr int kDigestThreads = (kConsumerWarps + kProducerWarps) * 32;
+static_assert(kConsumerWarps * kTM == kMT, "consumer warps must cover the row tile");
+
+// Warp-specialised, one CTA per SM: warps 0..7 (two warpgroups) are consumers -- LDS + DFMA only, thread tile
+// 16 x TN, warp w owns rows 16w..16w+15 and all 32 TN columns -- and warps 8..11 (one warpgroup) are producers:
+// panel index tables, cp.async of the A and B tiles into a 5-stage mbarrier ring.  setmaxnreg moves registers from
+// the producers (40) to the consumers (232).  The consumers never execute address arithmetic or CTA-wide barriers
+// (profiles/: in the first version the DFMA warps spent 27 % of their instructions on the loader and the fp64 pipe
+// stayed at 62 %).
 template <int TN>
-__global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
+__global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestArgs g)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     DigestSmem<TN>& S = *reinterpret_cast<DigestSmem<TN>*>(smem_raw);
@@ -77,11 +117,6 @@ __global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
     const int I = sc_.I, J = sc_.J;
     const int N = T.nao, nDp = g.nDp;
     const int nI = T.blk_nao[I], nJ = T.blk_nao[J];
-    // Warp w owns rows 8w..8w+7 of the CTA tile and all 32 TN columns (lane + 32 t): A is a broadcast LDS.128,
-    // B a conflict-free LDS.64.  (A 4 x 8 lane tiling was measured: same speed -- multicast LDS costs the same
-    // wavefronts -- and it cannot skip the warps of a ragged last row tile, which this mapping can.)
-    const int trow = w * 8;
-    const int tcol = lane;
     int R1, R2;                               // row blocks: constant over the run by construction
     switch (view) {
     case 0: R1 = I; R2 = J; break;
@@ -91,131 +126,158 @@ __global__ void __launch_bounds__(256, 2) digest_kernel(const DigestArgs g)
     case 4: R1 = I; R2 = it.a; break;
     default: R1 = J; R2 = it.a; break;
     }
-    const int nrows_all = T.blk_nao[R1] * T.blk_nao[R2];
-    const bool warp_active = it.rowtile * kMT + trow < nrows_all;   // ragged last tile: idle warps skip the DFMAs
+    const int nR2 = T.blk_nao[R2], nrows = T.blk_nao[R1] * nR2;
 
-    double acc[8][TN];
-#pragma unroll
-    for (int r = 0; r < 8; ++r)
-#pragma unroll
-        for (int t = 0; t < TN; ++t) acc[r][t] = 0.0;
+    if (tid == 0) {
+        for (int st = 0; st < kStages; ++st) {
+            mbar_init(&S.full[st], kProducerThreads);
+            mbar_init(&S.empty[st], kConsumerWarps);
+        }
+    }
+    __syncthreads();
 
-    const double* __restrict__ Bmat = (view <= 1) ? g.Dst : g.Dt;
-    const bool rowContig = (view == 1 || view >= 4);   // l (unit stride) is a row index
-
-    for (int s = 0; s < it.count; ++s) {
-        int K, L, rank;
+    // (K, L, rank) of step s of the run
+    auto step_blocks = [&](int s, int& K, int& L, int& rank) {
         if (view <= 1) { rank = it.a + s; K = T.pair_I[rank]; L = T.pair_J[rank]; }
         else if (view <= 3) { K = it.a; L = it.b + s; rank = T.rank_of[K * T.nblk + L]; }
         else { L = it.a; K = it.b + s; rank = T.rank_of[K * T.nblk + L]; }
-        const int nK = T.blk_nao[K], nL = T.blk_nao[L];
-        const double* __restrict__ P = g.panel + sc_.base + (T.koff[rank] - T.koff[sc_.r0]) * (long long)(nI * nJ);
-        const int sI = nJ * nK * nL, sJ = nK * nL, sK = nL, sL = 1;
-        int C1, C2, sR1, sR2, sC1, sC2;
+    };
+    // number of contraction columns of a step
+    auto step_cols = [&](int K, int L) {
         switch (view) {
-        case 0: C1 = K; C2 = L; sR1 = sI; sR2 = sJ; sC1 = sK; sC2 = sL; break;
-        case 1: C1 = I; C2 = J; sR1 = sK; sR2 = sL; sC1 = sI; sC2 = sJ; break;
-        case 2: C1 = J; C2 = L; sR1 = sI; sR2 = sK; sC1 = sJ; sC2 = sL; break;
-        case 3: C1 = I; C2 = L; sR1 = sJ; sR2 = sK; sC1 = sI; sC2 = sL; break;
-        case 4: C1 = J; C2 = K; sR1 = sI; sR2 = sL; sC1 = sJ; sC2 = sK; break;
-        default: C1 = I; C2 = K; sR1 = sJ; sR2 = sL; sC1 = sI; sC2 = sK; break;
+        case 0: return T.blk_nao[K] * T.blk_nao[L];
+        case 1: return nI * nJ;
+        case 2: return nJ * T.blk_nao[L];
+        case 3: return nI * T.blk_nao[L];
+        case 4: return nJ * T.blk_nao[K];
+        default: return nI * T.blk_nao[K];
         }
-        const int nR2 = T.blk_nao[R2], nrows = T.blk_nao[R1] * nR2;
-        const int nC2 = T.blk_nao[C2], nC = T.blk_nao[C1] * nC2;
-        const int aoC1 = T.blk_ao0[C1], aoC2 = T.blk_ao0[C2];
+    };
 
-        __syncthreads();   // previous step done with tables and stage buffers
-        if (tid < kMT) {
-            const int m = it.rowtile * kMT + tid;
-            S.rowoff[tid] = (m < nrows) ? (m / nR2) * sR1 + (m % nR2) * sR2 : -1;
+    if (w >= kConsumerWarps) {
+        // ===================== producer warpgroup =====================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
+        const int pt = tid - kConsumerWarps * 32, pw = pt >> 5;
+        const double* __restrict__ Bmat = (view <= 1) ? g.Dst : g.Dt;
+        const bool rowContig = (view == 1 || view >= 4);   // l (unit stride) is a row index
+        int gch = 0;
+        for (int s = 0; s < it.count; ++s) {
+            int K, L, rank;
+            step_blocks(s, K, L, rank);
+            const int nK = T.blk_nao[K], nL = T.blk_nao[L];
+            const double* __restrict__ P = g.panel + sc_.base + (T.koff[rank] - T.koff[sc_.r0]) * (long long)(nI * nJ);
+            const int sI = nJ * nK * nL, sJ = nK * nL, sK = nL, sL = 1;
+            int C1, C2, sR1, sR2, sC1, sC2;
+            switch (view) {
+            case 0: C1 = K; C2 = L; sR1 = sI; sR2 = sJ; sC1 = sK; sC2 = sL; break;
+            case 1: C1 = I; C2 = J; sR1 = sK; sR2 = sL; sC1 = sI; sC2 = sJ; break;
+            case 2: C1 = J; C2 = L; sR1 = sI; sR2 = sK; sC1 = sJ; sC2 = sL; break;
+            case 3: C1 = I; C2 = L; sR1 = sJ; sR2 = sK; sC1 = sI; sC2 = sL; break;
+            case 4: C1 = J; C2 = K; sR1 = sI; sR2 = sL; sC1 = sJ; sC2 = sK; break;
+            default: C1 = I; C2 = K; sR1 = sJ; sR2 = sL; sC1 = sI; sC2 = sK; break;
+            }
+            const int nC2 = T.blk_nao[C2], nC = T.blk_nao[C1] * nC2;
+            const int aoC1 = T.blk_ao0[C1], aoC2 = T.blk_ao0[C2];
+            asm volatile("bar.sync 1, %0;\n" ::"n"(kProducerThreads));   // previous panel's tables no longer read
+            {
+                const int mm = it.rowtile * kMT + pt;                     // kMT == kProducerThreads rows
+                S.rowoff[pt] = (mm < nrows) ? (mm / nR2) * sR1 + (mm % nR2) * sR2 : -1;
+            }
+            for (int cidx = pt; cidx < nC; cidx += kProducerThreads) {
+                const int c1 = cidx / nC2, c2 = cidx % nC2;
+                S.acol[cidx] = c1 * sC1 + c2 * sC2;
+                S.bcol[cidx] = partner ? (unsigned)((aoC2 + c2) * N + aoC1 + c1) : (unsigned)((aoC1 + c1) * N + aoC2 + c2);
+            }
+            asm volatile("bar.sync 1, %0;\n" ::"n"(kProducerThreads));
+            const int nch = (nC + kKC - 1) / kKC;
+            const int ro_fixed = S.rowoff[pt];                            // rowContig: this thread's row
+            for (int ch = 0; ch < nch; ++ch, ++gch) {
+                const int st = gch % kStages;
+                if (gch >= kStages) mbar_wait(&S.empty[st], (unsigned)((gch / kStages - 1) & 1));
+                // A tile: kKC x kMT elements of 8 bytes, 16 per producer thread, lanes along the unit-stride direction
+                if (rowContig) {
+#pragma unroll 4
+                    for (int k = 0; k < kKC; ++k) {
+                        const int cidx = ch * kKC + k;
+                        const bool ok = (ro_fixed >= 0) && (cidx < nC);
+                        cp_async8(&S.A[st][k][pt], ok ? (P + ro_fixed + S.acol[cidx]) : P, ok);
+                    }
+                } else {
+                    const int k = pt & 15, cidx = ch * kKC + k;
+                    const bool cok = cidx < nC;
+                    const int co = cok ? S.acol[cidx] : 0;
+#pragma unroll 4
+                    for (int e = 0; e < kMT / 8; ++e) {
+                        const int m = (pt >> 4) + 8 * e, ro = S.rowoff[m];
+                        const bool ok = cok && (ro >= 0);
+                        cp_async8(&S.A[st][k][m], ok ? (P + ro + co) : P, ok);
+                    }
+                }
+                // B tile: kKC density rows of 32 TN doubles, 16-byte pieces; warp pw copies rows pw, pw+4, ...
+#pragma unroll
+                for (int h = 0; h < kKC / kProducerWarps; ++h) {
+                    const int k = pw + kProducerWarps * h, cidx = ch * kKC + k;
+                    const bool ok = cidx < nC;
+                    const double* src = ok ? (Bmat + (size_t)S.bcol[cidx] * nDp + n0) : Bmat;
+                    for (int pc = lane; pc < 16 * TN; pc += 32) cp_async16(&S.B[st][k][pc * 2], src + (ok ? pc * 2 : 0), ok);
+                }
+                mbar_arrive_on_cp_async(&S.full[st]);
+            }
         }
-        for (int cidx = tid; cidx < nC; cidx += 256) {
-            const int c1 = cidx / nC2, c2 = cidx % nC2;
-            S.acol[cidx] = c1 * sC1 + c2 * sC2;
-            S.bcol[cidx] = partner ? (unsigned)((aoC2 + c2) * N + aoC1 + c1) : (unsigned)((aoC1 + c1) * N + aoC2 + c2);
-        }
-        __syncthreads();
+        return;
+    }
 
-        const int nch = (nC + kKC - 1) / kKC;
-        // Loader: everything that does not depend on the chunk is hoisted out of the chunk loop.
-        //   A tile (kKC x kMT doubles, 4 per thread): rowContig -> fixed row m, columns k = (tid>>6)+4e;
-        //                                             else      -> fixed column k, rows m = (tid>>4)+16e.
-        //   B tile: warp w copies rows k = w and w+8, lanes stride the 16-byte pieces of the row.
-        const int am = rowContig ? (tid & 63) : (tid >> 4);
-        const int ak = rowContig ? (tid >> 6) : (tid & 15);
-        int aro[4];
+    // ===================== consumer warpgroups =====================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
+    int total_chunks = 0;
+    for (int s = 0; s < it.count; ++s) {
+        int K, L, rank;
+        step_blocks(s, K, L, rank);
+        total_chunks += (step_cols(K, L) + kKC - 1) / kKC;
+    }
+    const int trow = w * kTM;
+    const bool warp_active = it.rowtile * kMT + trow < nrows;   // ragged last tile: idle warps skip the DFMAs
+    double acc[kTM][TN];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) aro[e] = S.rowoff[rowContig ? am : am + 16 * e];
-        auto load = [&](int st, int ch) {
-            if (rowContig) {
+    for (int r = 0; r < kTM; ++r)
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int k = ak + 4 * e, cidx = ch * kKC + k;
-                    const bool ok = (aro[0] >= 0) && (cidx < nC);
-                    cp_async8(&S.A[st][k][am], ok ? (P + aro[0] + S.acol[cidx]) : P, ok);
-                }
-            } else {
-                const int cidx = ch * kKC + ak;
-                const bool cok = cidx < nC;
-                const int co = cok ? S.acol[cidx] : 0;
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const bool ok = cok && (aro[e] >= 0);
-                    cp_async8(&S.A[st][ak][am + 16 * e], ok ? (P + aro[e] + co) : P, ok);
-                }
-            }
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int k = w + 8 * h, cidx = ch * kKC + k;
-                const bool ok = cidx < nC;
-                const double* src = ok ? (Bmat + (size_t)S.bcol[cidx] * nDp + n0) : Bmat;
-#pragma unroll
-                for (int pc = lane; pc < 16 * TN; pc += 32) cp_async16(&S.B[st][k][pc * 2], src + (ok ? pc * 2 : 0), ok);
-            }
-        };
-#pragma unroll
-        for (int st = 0; st < kStages - 1; ++st) {
-            if (st < nch) load(st, st);
-            cp_async_commit();
-        }
-        for (int ch = 0; ch < nch; ++ch) {
-            cp_async_wait<kStages - 2>();
-            __syncthreads();
-            const int nxt = ch + kStages - 1;
-            if (nxt < nch) load(nxt % kStages, nxt);
-            cp_async_commit();
-            const int st = ch % kStages;
-            if (warp_active) {
+        for (int t = 0; t < TN; ++t) acc[r][t] = 0.0;
+
+    for (int gch = 0; gch < total_chunks; ++gch) {
+        const int st = gch % kStages;
+        mbar_wait(&S.full[st], (unsigned)((gch / kStages) & 1));
+        if (warp_active) {
 #pragma unroll
             for (int k = 0; k < kKC; ++k) {
                 const double2* ap = reinterpret_cast<const double2*>(&S.A[st][k][trow]);
-                const double2 a01 = ap[0], a23 = ap[1], a45 = ap[2], a67 = ap[3];
-                const double a[8] = {a01.x, a01.y, a23.x, a23.y, a45.x, a45.y, a67.x, a67.y};
+                double a[kTM];
+#pragma unroll
+                for (int r = 0; r < kTM / 2; ++r) { const double2 v = ap[r]; a[2 * r] = v.x; a[2 * r + 1] = v.y; }
                 double b[TN];
 #pragma unroll
-                for (int t = 0; t < TN; ++t) b[t] = S.B[st][k][tcol + 32 * t];
+                for (int t = 0; t < TN; ++t) b[t] = S.B[st][k][lane + 32 * t];
 #pragma unroll
-                for (int r = 0; r < 8; ++r)
+                for (int r = 0; r < kTM; ++r)
 #pragma unroll
                     for (int t = 0; t < TN; ++t) acc[r][t] = fma(a[r], b[t], acc[r][t]);
             }
-            }
         }
-        cp_async_wait<0>();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&S.empty[st]);
     }
 
     // flush: coalesced fp64 reductions into the density-fastest accumulators
+    if (!warp_active) return;
     const double mult = (double)it.mult;
     double* __restrict__ Out = (view <= 1) ? g.Jt : g.Kt;
-    const int nR2 = T.blk_nao[R2], nrows = T.blk_nao[R1] * nR2;
     const int aoR1 = T.blk_ao0[R1], aoR2 = T.blk_ao0[R2];
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
+    for (int r = 0; r < kTM; ++r) {
         const int m = it.rowtile * kMT + trow + r;
         if (m < nrows) {
             const int r1 = m / nR2, r2 = m % nR2;
             const size_t row = partner ? (size_t)(aoR2 + r2) * N + aoR1 + r1 : (size_t)(aoR1 + r1) * N + aoR2 + r2;
-            double* o = Out + row * nDp + n0 + tcol;
+            double* o = Out + row * nDp + n0 + lane;
 #pragma unroll
             for (int t = 0; t < TN; ++t) atomicAdd(o + 32 * t, mult * acc[r][t]);
         }
@@ -231,7 +293,7 @@ static int launch_digest_tn(ltjk_ctx* c, const DigestArgs& g, int nitems, int nc
         LTJK_CUDA(c, cudaFuncSetAttribute(digest_kernel<TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    digest_kernel<TN><<<dim3(nitems, ncolblk), 256, smem, c->stream>>>(g);
+    digest_kernel<TN><<<dim3(nitems, ncolblk), kDigestThreads, smem, c->stream>>>(g);
     LTJK_CUDA(c, cudaGetLastError());
     return LTJK_OK;
 }

@@ -8,6 +8,8 @@
 
 namespace ltjk {
 
+constexpr int kDigestRows = 128;   // output rows per digestion CTA (ltjk_digest.cu) = row-tile height of the work items
+
 // ---- geometry-frozen device tables (built by ltjk_build_shell_pairs, reused by every jk_build) ----------------
 // Shells are re-ordered internally by angular momentum and cut into l-homogeneous BLOCKS of ~16 AOs; block
 // pairs (I>=J) are ranked class-major ((ss),(ps),(pp),(ds),(dp),(dd)), so that every canonical block quartet
