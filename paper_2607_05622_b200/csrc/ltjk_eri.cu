@@ -148,6 +148,12 @@ static int launch_cls(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
     if constexpr (CK <= CB) {
         const long long nthr = (long long)maxkets * g.qn;
         const int bs = 64;
+        static bool carve = false;      // no shared memory used: give the whole unified cache to L1 (local-memory spills)
+        if (!carve) {
+            cudaFuncSetAttribute(eri_panel_kernel<la[CB], lb[CB], la[CK], lb[CK]>,
+                                 cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxL1);
+            carve = true;
+        }
         eri_panel_kernel<la[CB], lb[CB], la[CK], lb[CK]>
             <<<dim3((unsigned)((nthr + bs - 1) / bs), nsub), bs, 0, c->eri_stream>>>(g);
         LTJK_CUDA(c, cudaGetLastError());
