@@ -78,8 +78,34 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
     long long used = 0;                                   // doubles used in the current ring half
     size_t j_first = 0;
     std::vector<DigestItem> jitems, kitems;
+    // contraction chunks of an item (the consumers of the digestion kernel need the count up front)
+    auto fill_chunks = [&](DigestItem& it) {
+        const SubChunk& sc = c->subs[it.sub];
+        const int nI = c->blk_nao[sc.I], nJ = c->blk_nao[sc.J];
+        int tot = 0;
+        for (int s = 0; s < it.count; ++s) {
+            int K, L;
+            if (it.view <= 1) { K = c->pair_I[it.a + s]; L = c->pair_J[it.a + s]; }
+            else if (it.view <= 3) { K = it.a; L = it.b + s; }
+            else { L = it.a; K = it.b + s; }
+            const int nK = c->blk_nao[K], nL = c->blk_nao[L];
+            int nC;
+            switch (it.view) {
+            case 0: nC = nK * nL; break;
+            case 1: nC = nI * nJ; break;
+            case 2: nC = nJ * nL; break;
+            case 3: nC = nI * nL; break;
+            case 4: nC = nJ * nK; break;
+            default: nC = nI * nK; break;
+            }
+            tot += (nC + 15) / 16;
+        }
+        it.nchunks = tot;
+    };
     auto close_group = [&]() {
         if (!open) return;
+        for (DigestItem& it : jitems) fill_chunks(it);
+        for (DigestItem& it : kitems) fill_chunks(it);
         auto longer = [](const DigestItem& a, const DigestItem& b) { return a.count > b.count; };
         std::stable_sort(jitems.begin(), jitems.end(), longer);      // longest runs first: shorter launch tail
         std::stable_sort(kitems.begin(), kitems.end(), longer);
@@ -128,12 +154,12 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
             for (int ra = r0; ra < r1; ra += kRunMax) {
                 const int cnt = std::min(kRunMax, r1 - ra);
                 for (int rt = 0; rt < rowtiles(nI * nJ); ++rt)
-                    jitems.push_back(DigestItem{0, 0, (unsigned char)rt, 1, ra, 0, cnt, sub});
+                    jitems.push_back(DigestItem{0, 0, (unsigned char)rt, 1, ra, 0, cnt, sub, 0});
             }
             for (int r = r0; r < r1; ++r) {
                 const int nK = c->blk_nao[c->pair_I[r]], nL = c->blk_nao[c->pair_J[r]];
                 for (int rt = 0; rt < rowtiles(nK * nL); ++rt)
-                    jitems.push_back(DigestItem{1, 0, (unsigned char)rt, 1, r, 0, 1, sub});
+                    jitems.push_back(DigestItem{1, 0, (unsigned char)rt, 1, r, 0, 1, sub, 0});
             }
             // ---- K views.  Diagonal block quartets: the panel is symmetric under i<->j when I == J and under
             // k<->l when K == L, which makes pairs of K images identical; they are digested once with weight 2:
@@ -144,7 +170,7 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
                 for (int partner = 0; partner < 2; ++partner)
                     for (int rt = 0; rt < rowtiles(rows); ++rt)
                         kitems.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned char)rt,
-                                                    (unsigned char)mult, fixed, first, cnt, sub});
+                                                    (unsigned char)mult, fixed, first, cnt, sub, 0});
             };
             // views 2,3: runs of consecutive ranks with the same K (L consecutive by construction); a K == L
             // panel ends the run it would belong to and is digested on its own with the extra weight

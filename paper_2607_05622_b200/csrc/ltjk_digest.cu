@@ -16,6 +16,7 @@
 // panels sharing that output block, and flushes once with coalesced fp64 reductions.
 #include "ltjk_internal.h"
 #include <cstdio>
+#include <algorithm>
 
 namespace ltjk {
 
@@ -96,37 +97,57 @@ constexpr int kProducerThreads = kProducerWarps * 32;
 constexpr int kDigestThreads = (kConsumerWarps + kProducerWarps) * 32;
 static_assert(kConsumerWarps * kTM == kMT, "consumer warps must cover the row tile");
 
-// Warp-specialised, one CTA per SM: warps 0..7 (two warpgroups) are consumers -- LDS + DFMA only, thread tile
-// 16 x TN, warp w owns rows 16w..16w+15 and all 32 TN columns -- and warps 8..11 (one warpgroup) are producers:
+// Warp-specialised, persistent, one CTA per SM: warps 0..7 (two warpgroups) are consumers -- LDS + DFMA only, thread
+// tile 16 x TN, warp w owns rows 16w..16w+15 and all 32 TN columns -- and warps 8..11 (one warpgroup) are producers:
 // panel index tables, cp.async of the A and B tiles into a 5-stage mbarrier ring.  setmaxnreg moves registers from
-// the producers (40) to the consumers (232).  The consumers never execute address arithmetic or CTA-wide barriers
-// (profiles/: in the first version the DFMA warps spent 27 % of their instructions on the loader and the fp64 pipe
-// stayed at 62 %).
+// the producers (40) to the consumers (232).  Every CTA walks the work items blockIdx.x, blockIdx.x + gridDim.x, ...;
+// the ring keeps running across items, so the producers prefetch the next item while the consumers finish and flush
+// the current one (profiles/: with one item per CTA the consumers idled ~15 % of the time at item starts; before
+// specialisation the DFMA warps spent 27 % of their instructions on the loader).
+struct ItemCtx {
+    DigestItem it;
+    SubChunk sc;
+    int R1, R2, nR2, nrows, nI, nJ, n0;
+};
+
+__device__ __forceinline__ ItemCtx load_item(const DigestArgs& g, int vi, int ncolblk, int colw)
+{
+    ItemCtx c;
+    const DevTables& T = g.t;
+    c.it = g.items[vi / ncolblk];
+    c.n0 = (vi % ncolblk) * colw;
+    c.sc = g.subs[c.it.sub];
+    const int I = c.sc.I, J = c.sc.J;
+    c.nI = T.blk_nao[I]; c.nJ = T.blk_nao[J];
+    switch (c.it.view) {                       // row blocks: constant over the run by construction
+    case 0: c.R1 = I; c.R2 = J; break;
+    case 1: c.R1 = T.pair_I[c.it.a]; c.R2 = T.pair_J[c.it.a]; break;
+    case 2: c.R1 = I; c.R2 = c.it.a; break;
+    case 3: c.R1 = J; c.R2 = c.it.a; break;
+    case 4: c.R1 = I; c.R2 = c.it.a; break;
+    default: c.R1 = J; c.R2 = c.it.a; break;
+    }
+    c.nR2 = T.blk_nao[c.R2];
+    c.nrows = T.blk_nao[c.R1] * c.nR2;
+    return c;
+}
+
+// (K, L, rank) of step s of the run
+__device__ __forceinline__ void step_blocks(const DevTables& T, const DigestItem& it, int s, int& K, int& L, int& rank)
+{
+    if (it.view <= 1) { rank = it.a + s; K = T.pair_I[rank]; L = T.pair_J[rank]; }
+    else if (it.view <= 3) { K = it.a; L = it.b + s; rank = T.rank_of[K * T.nblk + L]; }
+    else { L = it.a; K = it.b + s; rank = T.rank_of[K * T.nblk + L]; }
+}
+
 template <int TN>
-__global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestArgs g)
+__global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestArgs g, const int nvirt, const int ncolblk)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     DigestSmem<TN>& S = *reinterpret_cast<DigestSmem<TN>*>(smem_raw);
     const DevTables& T = g.t;
-    const DigestItem it = g.items[blockIdx.x];
-    const int n0 = blockIdx.y * (32 * TN);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int view = it.view;
-    const bool partner = it.partner != 0;
-    const SubChunk sc_ = g.subs[it.sub];
-    const int I = sc_.I, J = sc_.J;
     const int N = T.nao, nDp = g.nDp;
-    const int nI = T.blk_nao[I], nJ = T.blk_nao[J];
-    int R1, R2;                               // row blocks: constant over the run by construction
-    switch (view) {
-    case 0: R1 = I; R2 = J; break;
-    case 1: R1 = T.pair_I[it.a]; R2 = T.pair_J[it.a]; break;
-    case 2: R1 = I; R2 = it.a; break;
-    case 3: R1 = J; R2 = it.a; break;
-    case 4: R1 = I; R2 = it.a; break;
-    default: R1 = J; R2 = it.a; break;
-    }
-    const int nR2 = T.blk_nao[R2], nrows = T.blk_nao[R1] * nR2;
 
     if (tid == 0) {
         for (int st = 0; st < kStages; ++st) {
@@ -135,93 +156,82 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
         }
     }
     __syncthreads();
-
-    // (K, L, rank) of step s of the run
-    auto step_blocks = [&](int s, int& K, int& L, int& rank) {
-        if (view <= 1) { rank = it.a + s; K = T.pair_I[rank]; L = T.pair_J[rank]; }
-        else if (view <= 3) { K = it.a; L = it.b + s; rank = T.rank_of[K * T.nblk + L]; }
-        else { L = it.a; K = it.b + s; rank = T.rank_of[K * T.nblk + L]; }
-    };
-    // number of contraction columns of a step
-    auto step_cols = [&](int K, int L) {
-        switch (view) {
-        case 0: return T.blk_nao[K] * T.blk_nao[L];
-        case 1: return nI * nJ;
-        case 2: return nJ * T.blk_nao[L];
-        case 3: return nI * T.blk_nao[L];
-        case 4: return nJ * T.blk_nao[K];
-        default: return nI * T.blk_nao[K];
-        }
-    };
+    int gch = 0;                                   // chunk counter of the ring, runs across items in both roles
 
     if (w >= kConsumerWarps) {
         // ===================== producer warpgroup =====================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
         const int pt = tid - kConsumerWarps * 32, pw = pt >> 5;
-        const double* __restrict__ Bmat = (view <= 1) ? g.Dst : g.Dt;
-        const bool rowContig = (view == 1 || view >= 4);   // l (unit stride) is a row index
-        int gch = 0;
-        for (int s = 0; s < it.count; ++s) {
-            int K, L, rank;
-            step_blocks(s, K, L, rank);
-            const int nK = T.blk_nao[K], nL = T.blk_nao[L];
-            const double* __restrict__ P = g.panel + sc_.base + (T.koff[rank] - T.koff[sc_.r0]) * (long long)(nI * nJ);
-            const int sI = nJ * nK * nL, sJ = nK * nL, sK = nL, sL = 1;
-            int C1, C2, sR1, sR2, sC1, sC2;
-            switch (view) {
-            case 0: C1 = K; C2 = L; sR1 = sI; sR2 = sJ; sC1 = sK; sC2 = sL; break;
-            case 1: C1 = I; C2 = J; sR1 = sK; sR2 = sL; sC1 = sI; sC2 = sJ; break;
-            case 2: C1 = J; C2 = L; sR1 = sI; sR2 = sK; sC1 = sJ; sC2 = sL; break;
-            case 3: C1 = I; C2 = L; sR1 = sJ; sR2 = sK; sC1 = sI; sC2 = sL; break;
-            case 4: C1 = J; C2 = K; sR1 = sI; sR2 = sL; sC1 = sJ; sC2 = sK; break;
-            default: C1 = I; C2 = K; sR1 = sJ; sR2 = sL; sC1 = sI; sC2 = sK; break;
-            }
-            const int nC2 = T.blk_nao[C2], nC = T.blk_nao[C1] * nC2;
-            const int aoC1 = T.blk_ao0[C1], aoC2 = T.blk_ao0[C2];
-            asm volatile("bar.sync 1, %0;\n" ::"n"(kProducerThreads));   // previous panel's tables no longer read
-            {
-                const int mm = it.rowtile * kMT + pt;                     // kMT == kProducerThreads rows
-                S.rowoff[pt] = (mm < nrows) ? (mm / nR2) * sR1 + (mm % nR2) * sR2 : -1;
-            }
-            for (int cidx = pt; cidx < nC; cidx += kProducerThreads) {
-                const int c1 = cidx / nC2, c2 = cidx % nC2;
-                S.acol[cidx] = c1 * sC1 + c2 * sC2;
-                S.bcol[cidx] = partner ? (unsigned)((aoC2 + c2) * N + aoC1 + c1) : (unsigned)((aoC1 + c1) * N + aoC2 + c2);
-            }
-            asm volatile("bar.sync 1, %0;\n" ::"n"(kProducerThreads));
-            const int nch = (nC + kKC - 1) / kKC;
-            const int ro_fixed = S.rowoff[pt];                            // rowContig: this thread's row
-            for (int ch = 0; ch < nch; ++ch, ++gch) {
-                const int st = gch % kStages;
-                if (gch >= kStages) mbar_wait(&S.empty[st], (unsigned)((gch / kStages - 1) & 1));
-                // A tile: kKC x kMT elements of 8 bytes, 16 per producer thread, lanes along the unit-stride direction
-                if (rowContig) {
-#pragma unroll 4
-                    for (int k = 0; k < kKC; ++k) {
-                        const int cidx = ch * kKC + k;
-                        const bool ok = (ro_fixed >= 0) && (cidx < nC);
-                        cp_async8(&S.A[st][k][pt], ok ? (P + ro_fixed + S.acol[cidx]) : P, ok);
-                    }
-                } else {
-                    const int k = pt & 15, cidx = ch * kKC + k;
-                    const bool cok = cidx < nC;
-                    const int co = cok ? S.acol[cidx] : 0;
-#pragma unroll 4
-                    for (int e = 0; e < kMT / 8; ++e) {
-                        const int m = (pt >> 4) + 8 * e, ro = S.rowoff[m];
-                        const bool ok = cok && (ro >= 0);
-                        cp_async8(&S.A[st][k][m], ok ? (P + ro + co) : P, ok);
-                    }
+        for (int vi = blockIdx.x; vi < nvirt; vi += gridDim.x) {
+            const ItemCtx c = load_item(g, vi, ncolblk, 32 * TN);
+            const DigestItem& it = c.it;
+            const int view = it.view, I = c.sc.I, J = c.sc.J, nI = c.nI, nJ = c.nJ;
+            const bool partner = it.partner != 0;
+            const double* __restrict__ Bmat = (view <= 1) ? g.Dst : g.Dt;
+            const bool rowContig = (view == 1 || view >= 4);   // l (unit stride) is a row index
+            for (int s = 0; s < it.count; ++s) {
+                int K, L, rank;
+                step_blocks(T, it, s, K, L, rank);
+                const int nK = T.blk_nao[K], nL = T.blk_nao[L];
+                const double* __restrict__ P = g.panel + c.sc.base + (T.koff[rank] - T.koff[c.sc.r0]) * (long long)(nI * nJ);
+                const int sI = nJ * nK * nL, sJ = nK * nL, sK = nL, sL = 1;
+                int C1, C2, sR1, sR2, sC1, sC2;
+                switch (view) {
+                case 0: C1 = K; C2 = L; sR1 = sI; sR2 = sJ; sC1 = sK; sC2 = sL; break;
+                case 1: C1 = I; C2 = J; sR1 = sK; sR2 = sL; sC1 = sI; sC2 = sJ; break;
+                case 2: C1 = J; C2 = L; sR1 = sI; sR2 = sK; sC1 = sJ; sC2 = sL; break;
+                case 3: C1 = I; C2 = L; sR1 = sJ; sR2 = sK; sC1 = sI; sC2 = sL; break;
+                case 4: C1 = J; C2 = K; sR1 = sI; sR2 = sL; sC1 = sJ; sC2 = sK; break;
+                default: C1 = I; C2 = K; sR1 = sJ; sR2 = sL; sC1 = sI; sC2 = sK; break;
                 }
-                // B tile: kKC density rows of 32 TN doubles, 16-byte pieces; warp pw copies rows pw, pw+4, ...
+                const int nC2 = T.blk_nao[C2], nC = T.blk_nao[C1] * nC2;
+                const int aoC1 = T.blk_ao0[C1], aoC2 = T.blk_ao0[C2];
+                asm volatile("bar.sync 1, %0;\n" ::"n"(kProducerThreads));   // previous panel's tables no longer read
+                {
+                    const int mm = it.rowtile * kMT + pt;                     // kMT == kProducerThreads rows
+                    S.rowoff[pt] = (mm < c.nrows) ? (mm / c.nR2) * sR1 + (mm % c.nR2) * sR2 : -1;
+                }
+                for (int cidx = pt; cidx < nC; cidx += kProducerThreads) {
+                    const int c1 = cidx / nC2, c2 = cidx % nC2;
+                    S.acol[cidx] = c1 * sC1 + c2 * sC2;
+                    S.bcol[cidx] = partner ? (unsigned)((aoC2 + c2) * N + aoC1 + c1) : (unsigned)((aoC1 + c1) * N + aoC2 + c2);
+                }
+                asm volatile("bar.sync 1, %0;\n" ::"n"(kProducerThreads));
+                const int nch = (nC + kKC - 1) / kKC;
+                const int ro_fixed = S.rowoff[pt];                            // rowContig: this thread's row
+                for (int ch = 0; ch < nch; ++ch, ++gch) {
+                    const int st = gch % kStages;
+                    if (gch >= kStages) mbar_wait(&S.empty[st], (unsigned)((gch / kStages - 1) & 1));
+                    // A tile: kKC x kMT elements of 8 bytes, 16 per producer thread, lanes along the unit stride
+                    if (rowContig) {
+#pragma unroll 4
+                        for (int k = 0; k < kKC; ++k) {
+                            const int cidx = ch * kKC + k;
+                            const bool ok = (ro_fixed >= 0) && (cidx < nC);
+                            cp_async8(&S.A[st][k][pt], ok ? (P + ro_fixed + S.acol[cidx]) : P, ok);
+                        }
+                    } else {
+                        const int k = pt & 15, cidx = ch * kKC + k;
+                        const bool cok = cidx < nC;
+                        const int co = cok ? S.acol[cidx] : 0;
+#pragma unroll 4
+                        for (int e = 0; e < kMT / 8; ++e) {
+                            const int m = (pt >> 4) + 8 * e, ro = S.rowoff[m];
+                            const bool ok = cok && (ro >= 0);
+                            cp_async8(&S.A[st][k][m], ok ? (P + ro + co) : P, ok);
+                        }
+                    }
+                    // B tile: kKC density rows of 32 TN doubles, 16-byte pieces; warp pw copies rows pw, pw+4, ...
 #pragma unroll
-                for (int h = 0; h < kKC / kProducerWarps; ++h) {
-                    const int k = pw + kProducerWarps * h, cidx = ch * kKC + k;
-                    const bool ok = cidx < nC;
-                    const double* src = ok ? (Bmat + (size_t)S.bcol[cidx] * nDp + n0) : Bmat;
-                    for (int pc = lane; pc < 16 * TN; pc += 32) cp_async16(&S.B[st][k][pc * 2], src + (ok ? pc * 2 : 0), ok);
+                    for (int h = 0; h < kKC / kProducerWarps; ++h) {
+                        const int k = pw + kProducerWarps * h, cidx = ch * kKC + k;
+                        const bool ok = cidx < nC;
+                        const double* src = ok ? (Bmat + (size_t)S.bcol[cidx] * nDp + c.n0) : Bmat;
+                        for (int pc = lane; pc < 16 * TN; pc += 32)
+                            cp_async16(&S.B[st][k][pc * 2], src + (ok ? pc * 2 : 0), ok);
+                    }
+                    mbar_arrive_on_cp_async(&S.full[st]);
                 }
-                mbar_arrive_on_cp_async(&S.full[st]);
             }
         }
         return;
@@ -229,57 +239,59 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
 
     // ===================== consumer warpgroups =====================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
-    int total_chunks = 0;
-    for (int s = 0; s < it.count; ++s) {
-        int K, L, rank;
-        step_blocks(s, K, L, rank);
-        total_chunks += (step_cols(K, L) + kKC - 1) / kKC;
-    }
     const int trow = w * kTM;
-    const bool warp_active = it.rowtile * kMT + trow < nrows;   // ragged last tile: idle warps skip the DFMAs
-    double acc[kTM][TN];
+    for (int vi = blockIdx.x; vi < nvirt; vi += gridDim.x) {
+        const ItemCtx c = load_item(g, vi, ncolblk, 32 * TN);
+        const DigestItem& it = c.it;
+        const int view = it.view;
+        const int total_chunks = it.nchunks;
+        const bool warp_active = it.rowtile * kMT + trow < c.nrows;   // ragged last tile: idle warps skip the DFMAs
+        double acc[kTM][TN];
 #pragma unroll
-    for (int r = 0; r < kTM; ++r)
+        for (int r = 0; r < kTM; ++r)
 #pragma unroll
-        for (int t = 0; t < TN; ++t) acc[r][t] = 0.0;
+            for (int t = 0; t < TN; ++t) acc[r][t] = 0.0;
 
-    for (int gch = 0; gch < total_chunks; ++gch) {
-        const int st = gch % kStages;
-        mbar_wait(&S.full[st], (unsigned)((gch / kStages) & 1));
-        if (warp_active) {
+        for (int q = 0; q < total_chunks; ++q, ++gch) {
+            const int st = gch % kStages;
+            mbar_wait(&S.full[st], (unsigned)((gch / kStages) & 1));
+            if (warp_active) {
 #pragma unroll
-            for (int k = 0; k < kKC; ++k) {
-                const double2* ap = reinterpret_cast<const double2*>(&S.A[st][k][trow]);
-                double a[kTM];
+                for (int k = 0; k < kKC; ++k) {
+                    const double2* ap = reinterpret_cast<const double2*>(&S.A[st][k][trow]);
+                    double a[kTM];
 #pragma unroll
-                for (int r = 0; r < kTM / 2; ++r) { const double2 v = ap[r]; a[2 * r] = v.x; a[2 * r + 1] = v.y; }
-                double b[TN];
+                    for (int r = 0; r < kTM / 2; ++r) { const double2 v = ap[r]; a[2 * r] = v.x; a[2 * r + 1] = v.y; }
+                    double b[TN];
 #pragma unroll
-                for (int t = 0; t < TN; ++t) b[t] = S.B[st][k][lane + 32 * t];
+                    for (int t = 0; t < TN; ++t) b[t] = S.B[st][k][lane + 32 * t];
 #pragma unroll
-                for (int r = 0; r < kTM; ++r)
+                    for (int r = 0; r < kTM; ++r)
 #pragma unroll
-                    for (int t = 0; t < TN; ++t) acc[r][t] = fma(a[r], b[t], acc[r][t]);
+                        for (int t = 0; t < TN; ++t) acc[r][t] = fma(a[r], b[t], acc[r][t]);
+                }
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&S.empty[st]);
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&S.empty[st]);
-    }
 
-    // flush: coalesced fp64 reductions into the density-fastest accumulators
-    if (!warp_active) return;
-    const double mult = (double)it.mult;
-    double* __restrict__ Out = (view <= 1) ? g.Jt : g.Kt;
-    const int aoR1 = T.blk_ao0[R1], aoR2 = T.blk_ao0[R2];
+        // flush: coalesced fp64 reductions into the density-fastest accumulators
+        if (warp_active) {
+            const double mult = (double)it.mult;
+            const bool partner = it.partner != 0;
+            double* __restrict__ Out = (view <= 1) ? g.Jt : g.Kt;
+            const int aoR1 = T.blk_ao0[c.R1], aoR2 = T.blk_ao0[c.R2];
 #pragma unroll
-    for (int r = 0; r < kTM; ++r) {
-        const int m = it.rowtile * kMT + trow + r;
-        if (m < nrows) {
-            const int r1 = m / nR2, r2 = m % nR2;
-            const size_t row = partner ? (size_t)(aoR2 + r2) * N + aoR1 + r1 : (size_t)(aoR1 + r1) * N + aoR2 + r2;
-            double* o = Out + row * nDp + n0 + lane;
+            for (int r = 0; r < kTM; ++r) {
+                const int m = it.rowtile * kMT + trow + r;
+                if (m < c.nrows) {
+                    const int r1 = m / c.nR2, r2 = m % c.nR2;
+                    const size_t row = partner ? (size_t)(aoR2 + r2) * N + aoR1 + r1 : (size_t)(aoR1 + r1) * N + aoR2 + r2;
+                    double* o = Out + row * nDp + c.n0 + lane;
 #pragma unroll
-            for (int t = 0; t < TN; ++t) atomicAdd(o + 32 * t, mult * acc[r][t]);
+                    for (int t = 0; t < TN; ++t) atomicAdd(o + 32 * t, mult * acc[r][t]);
+                }
+            }
         }
     }
 }
@@ -293,7 +305,12 @@ static int launch_digest_tn(ltjk_ctx* c, const DigestArgs& g, int nitems, int nc
         LTJK_CUDA(c, cudaFuncSetAttribute(digest_kernel<TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    digest_kernel<TN><<<dim3(nitems, ncolblk), kDigestThreads, smem, c->stream>>>(g);
+    int dev = 0, nsm = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    const long long nvirt = (long long)nitems * ncolblk;
+    const int grid = (int)std::min<long long>(nvirt, 8ll * nsm);   // 8 persistent waves: coarse dynamic balance, few start-up bubbles
+    digest_kernel<TN><<<grid, kDigestThreads, smem, c->stream>>>(g, (int)nvirt, ncolblk);
     LTJK_CUDA(c, cudaGetLastError());
     return LTJK_OK;
 }

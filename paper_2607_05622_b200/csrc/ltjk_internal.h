@@ -41,7 +41,7 @@ struct SubChunk {
     long long base;         // offset (doubles) of the first panel inside the ring half
 };
 
-// One digestion work item (20 bytes): a row tile of one output block accumulated over a run of panels.
+// One digestion work item (24 bytes): a row tile of one output block accumulated over a run of panels.
 struct DigestItem {
     unsigned char view;     // 0 JIJ, 1 JKL, 2 KIK, 3 KJK, 4 KIL, 5 KJL
     unsigned char partner;  // K views: 0 -> K[(r1,r2)] with D[(c1,c2)];  1 -> K[(r2,r1)] with D[(c2,c1)]
@@ -51,6 +51,7 @@ struct DigestItem {
     int b;                  // KIK/KJK: first L;  KIL/KJL: first K
     int count;              // panels in the run
     int sub;                // sub-chunk (global index)
+    int nchunks;            // contraction chunks (of 16 columns) over the whole run: sum over panels of ceil(nC/16)
 };
 
 // A group: consecutive sub-chunks of one bra class that fit one ring half; one ERI launch per ket class and one
