@@ -1,6 +1,6 @@
 // ltjk_transform.cu -- step a4: Laplace pseudo-densities (Eqs. 13-15; Alg. 1 lines 5-7)
 //   D^{alpha,d} = (C_o e^{+eps_o tau_alpha}) T_d (C_v e^{-eps_v tau_alpha})^T
-// evaluated as two batched fp64 GEMMs per (alpha, d):
+// evaluated as two batched fp64 tensor-core (DMMA) GEMMs per (alpha, d):
 //   W = [e^{(eps_i - eps_b) tau} T_d[i][b]] . C_v^T      (nocc x N)      -- the exponentials are fused into the load
 //   D = C_o . W                                          (N x N)
 // (nocc < nvir, so contracting the virtual index first is the cheaper order.)
@@ -34,12 +34,24 @@ struct GemmArgs {
     int nzb;
 };
 
+// FP64 tensor cores (DMMA): mma.sync m8n8k4, A row-major 8x4 (1 double per lane), B column-major 4x8, C 8x8
+// (2 doubles per lane).  This is the only place the path uses tensor cores (north_star: "FP64 tensor cores are used
+// only for the dense pseudo-density GEMMs"); tcgen05 has no f64 kind, so the Blackwell fp64 tensor path is mma.sync.
+__device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, const double a, const double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+// CTA tile 64 x 64, 8 warps as 2 x 4, warp tile 32 x 16 = 4 x 2 DMMA tiles, K step 16 through shared memory
+// (row stride 68 doubles: the 16 lanes of a half-warp -- 4 k x 4 m -- then fall into 16 different 8-byte banks).
 template <bool TRANSB>
 __global__ void __launch_bounds__(256) gemm_kernel(const GemmArgs g)
 {
-    constexpr int BM = 64, BN = 64, BK = 16;
-    __shared__ double As[BK][BM + 2];
-    __shared__ double Bs[BK][BN + 2];
+    constexpr int BM = 64, BN = 64, BK = 16, LD = 68;
+    __shared__ double As[BK][LD];
+    __shared__ double Bs[BK][LD];
     const int za = blockIdx.z / g.nzb, zb = blockIdx.z % g.nzb;
     const double* __restrict__ A = g.A + za * g.sAa + zb * g.sAb;
     const double* __restrict__ B = g.B + za * g.sBa + zb * g.sBb;
@@ -47,8 +59,10 @@ __global__ void __launch_bounds__(256) gemm_kernel(const GemmArgs g)
     const double* sr = g.sr ? g.sr + za * g.ssr : nullptr;
     const double* sc = g.sc ? g.sc + za * g.ssc : nullptr;
     const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
-    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-    double acc[4][4] = {};
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int wm = (w >> 2) * 32, wn = (w & 3) * 16;
+    const int lr = lane >> 2, lk = lane & 3;
+    double acc[4][2][2] = {};
     for (int k0 = 0; k0 < g.K; k0 += BK) {
         // A tile: 64 x 16, lanes along k (contiguous)
 #pragma unroll
@@ -79,27 +93,28 @@ __global__ void __launch_bounds__(256) gemm_kernel(const GemmArgs g)
         }
         __syncthreads();
 #pragma unroll
-        for (int k = 0; k < BK; ++k) {
-            double a[4], b[4];
+        for (int k4 = 0; k4 < BK; k4 += 4) {
+            double a[4], b[2];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) a[i] = As[k][ty * 4 + i];
+            for (int i = 0; i < 4; ++i) a[i] = As[k4 + lk][wm + 8 * i + lr];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) b[j] = Bs[k][tx + 16 * j];
+            for (int j = 0; j < 2; ++j) b[j] = Bs[k4 + lk][wn + 8 * j + lr];
 #pragma unroll
             for (int i = 0; i < 4; ++i)
 #pragma unroll
-                for (int j = 0; j < 4; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+                for (int j = 0; j < 2; ++j) dmma_m8n8k4(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
         __syncthreads();
     }
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const int gm = m0 + ty * 4 + i;
+        const int gm = m0 + wm + 8 * i + lr;
         if (gm >= g.M) continue;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int gn = n0 + tx + 16 * j;
-            if (gn < g.Nn) C[(size_t)gm * g.Nn + gn] = acc[i][j];
+        for (int j = 0; j < 2; ++j) {
+            const int gn = n0 + wn + 8 * j + 2 * lk;
+            if (gn < g.Nn) C[(size_t)gm * g.Nn + gn] = acc[i][j][0];
+            if (gn + 1 < g.Nn) C[(size_t)gm * g.Nn + gn + 1] = acc[i][j][1];
         }
     }
 }
