@@ -35,12 +35,12 @@ void free_tables(ltjk_ctx* c)
 {
     DevTables& t = c->t;
     void* ptrs[] = {t.pair_rec, t.schwarz, t.sh_ao, t.blk_sh0, t.blk_nsh, t.blk_ao0, t.blk_nao, t.pair_I, t.pair_J,
-                    t.koff, t.rank_of, t.ao_perm, c->d_items, c->d_subs, c->d_panel};
+                    t.koff, t.rank_of, t.ao_perm, t.ao_sh, c->d_items, c->d_subs, c->d_chunkmask, c->d_panel};
     for (void* p : ptrs) if (p) cudaFree(p);
     double* boys = t.boys;
     t = DevTables();
     t.boys = boys;
-    c->d_items = nullptr; c->d_subs = nullptr; c->d_panel = nullptr; c->panel_cap = 0; c->panel_half = 0; c->n_items = 0;
+    c->d_items = nullptr; c->d_subs = nullptr; c->d_chunkmask = nullptr; c->n_maskbits = 0; c->d_panel = nullptr; c->panel_cap = 0; c->panel_half = 0; c->n_items = 0;
     c->have_pairs = false;
 }
 
@@ -154,12 +154,12 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
             for (int ra = r0; ra < r1; ra += kRunMax) {
                 const int cnt = std::min(kRunMax, r1 - ra);
                 for (int rt = 0; rt < rowtiles(nI * nJ); ++rt)
-                    jitems.push_back(DigestItem{0, 0, (unsigned char)rt, 1, ra, 0, cnt, sub, 0});
+                    jitems.push_back(DigestItem{0, 0, (unsigned char)rt, 1, ra, 0, cnt, sub, 0, 0, 0u});
             }
             for (int r = r0; r < r1; ++r) {
                 const int nK = c->blk_nao[c->pair_I[r]], nL = c->blk_nao[c->pair_J[r]];
                 for (int rt = 0; rt < rowtiles(nK * nL); ++rt)
-                    jitems.push_back(DigestItem{1, 0, (unsigned char)rt, 1, r, 0, 1, sub, 0});
+                    jitems.push_back(DigestItem{1, 0, (unsigned char)rt, 1, r, 0, 1, sub, 0, 0, 0u});
             }
             // ---- K views.  Diagonal block quartets: the panel is symmetric under i<->j when I == J and under
             // k<->l when K == L, which makes pairs of K images identical; they are digested once with weight 2:
@@ -170,7 +170,7 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
                 for (int partner = 0; partner < 2; ++partner)
                     for (int rt = 0; rt < rowtiles(rows); ++rt)
                         kitems.push_back(DigestItem{(unsigned char)view, (unsigned char)partner, (unsigned char)rt,
-                                                    (unsigned char)mult, fixed, first, cnt, sub, 0});
+                                                    (unsigned char)mult, fixed, first, cnt, sub, 0, 0, 0u});
             };
             // views 2,3: runs of consecutive ranks with the same K (L consecutive by construction); a K == L
             // panel ends the run it would belong to and is digested on its own with the extra weight

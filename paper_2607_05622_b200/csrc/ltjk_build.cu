@@ -147,13 +147,30 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     std::vector<DigestItem> items;
     build_work(c, items);
     c->n_items = (long long)items.size();
+    {   // chunk mask layout: partner items of one tile share nothing here; one bit per (item, chunk)
+        unsigned long long bits = 0;
+        for (DigestItem& it : items) {
+            if (bits + (unsigned long long)it.nchunks >= 0xffffffffull)
+                return set_err(c, LTJK_ENOMEM, "build_shell_pairs: chunk mask exceeds 2^32 bits");
+            it.maskoff = (unsigned)bits; it.nnz = it.nchunks;
+            bits += (unsigned long long)it.nchunks;
+        }
+        c->n_maskbits = (long long)bits;
+    }
+    std::vector<int> ao_sh(c->nao, 0);
+    for (int s = 0; s < ns; ++s) {
+        const int n = ncart(c->l[c->sh_int2ext[s]]);
+        for (int k = 0; k < n; ++k) ao_sh[c->sh_ao_int[s] + k] = s;
+    }
     if ((rc = upload(c, &c->d_items, items)) || (rc = upload(c, &c->d_subs, c->subs)) || (rc = upload(c, &t.sh_ao, c->sh_ao_int)) ||
         (rc = upload(c, &t.blk_sh0, c->blk_sh0)) || (rc = upload(c, &t.blk_nsh, c->blk_nsh)) ||
         (rc = upload(c, &t.blk_ao0, c->blk_ao0)) || (rc = upload(c, &t.blk_nao, c->blk_nao)) ||
         (rc = upload(c, &t.pair_I, c->pair_I)) || (rc = upload(c, &t.pair_J, c->pair_J)) ||
         (rc = upload(c, &t.koff, c->koff)) || (rc = upload(c, &t.rank_of, c->rank_of)) ||
-        (rc = upload(c, &t.ao_perm, c->ao_perm)))
+        (rc = upload(c, &t.ao_perm, c->ao_perm)) || (rc = upload(c, &t.ao_sh, ao_sh)))
         return rc;
+    LTJK_CUDA(c, cudaMalloc(&c->d_chunkmask, sizeof(unsigned) * (size_t)(c->n_maskbits / 32 + 2)));
+    if ((rc = launch_chunk_mask(c))) return rc;
     LTJK_CUDA(c, cudaStreamSynchronize(c->stream));
     c->have_pairs = true;
     if (n_pairs) *n_pairs = (long long)ns * (ns + 1) / 2;

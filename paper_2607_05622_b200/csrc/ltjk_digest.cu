@@ -34,6 +34,7 @@ struct DigestArgs {
     const double* panel;
     const double* Dt;
     const double* Dst;
+    const unsigned* mask;
     double* Jt;
     double* Kt;
     int nDp;
@@ -169,6 +170,7 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
             const bool partner = it.partner != 0;
             const double* __restrict__ Bmat = (view <= 1) ? g.Dst : g.Dt;
             const bool rowContig = (view == 1 || view >= 4);   // l (unit stride) is a row index
+            int qi = 0;                                        // chunk index inside the item (mask position)
             for (int s = 0; s < it.count; ++s) {
                 int K, L, rank;
                 step_blocks(T, it, s, K, L, rank);
@@ -199,7 +201,10 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
                 asm volatile("bar.sync 1, %0;\n" ::"n"(kProducerThreads));
                 const int nch = (nC + kKC - 1) / kKC;
                 const int ro_fixed = S.rowoff[pt];                            // rowContig: this thread's row
-                for (int ch = 0; ch < nch; ++ch, ++gch) {
+                for (int ch = 0; ch < nch; ++ch, ++qi) {
+                    // tiles whose integrals are all Schwarz-screened (exact zeros in the panel) are never loaded
+                    const unsigned bit = it.maskoff + (unsigned)qi;
+                    if (!((g.mask[bit >> 5] >> (bit & 31u)) & 1u)) continue;
                     const int st = gch % kStages;
                     if (gch >= kStages) mbar_wait(&S.empty[st], (unsigned)((gch / kStages - 1) & 1));
                     // A tile: kKC x kMT elements of 8 bytes, 16 per producer thread, lanes along the unit stride
@@ -231,6 +236,7 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
                             cp_async16(&S.B[st][k][pc * 2], src + (ok ? pc * 2 : 0), ok);
                     }
                     mbar_arrive_on_cp_async(&S.full[st]);
+                    ++gch;
                 }
             }
         }
@@ -244,7 +250,7 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
         const ItemCtx c = load_item(g, vi, ncolblk, 32 * TN);
         const DigestItem& it = c.it;
         const int view = it.view;
-        const int total_chunks = it.nchunks;
+        const int total_chunks = it.nnz;
         const bool warp_active = it.rowtile * kMT + trow < c.nrows;   // ragged last tile: idle warps skip the DFMAs
         double acc[kTM][TN];
 #pragma unroll
@@ -334,7 +340,7 @@ int launch_digest(ltjk_ctx* c, const Group& ch, int nDp, bool doJ, bool doK)
     const int nitems = (doJ ? ch.nitemsJ : 0) + (doK ? ch.nitemsK : 0);
     if (nitems == 0) return LTJK_OK;
     DigestArgs g;
-    g.t = c->t; g.items = c->d_items + first; g.subs = c->d_subs; g.panel = c->d_panel + (size_t)ch.buf * c->panel_half;
+    g.t = c->t; g.items = c->d_items + first; g.subs = c->d_subs; g.mask = c->d_chunkmask; g.panel = c->d_panel + (size_t)ch.buf * c->panel_half;
     g.Dt = c->Dt; g.Dst = c->Dst; g.Jt = c->Jt; g.Kt = c->Kt;
     g.nDp = nDp;
     int TN, nb;
@@ -349,6 +355,99 @@ int launch_digest(ltjk_ctx* c, const Group& ch, int nDp, bool doJ, bool doK)
     case 5: return launch_digest_tn<5>(c, g, nitems, nb);
     default: return launch_digest_tn<6>(c, g, nitems, nb);
     }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a5, geometry-frozen: for every work item and every contraction chunk, does the 128 x 16 tile of the panel view hold
+// at least one integral of an unscreened shell quartet (Q_ij Q_kl >= tau)?  One CTA per item, threads over chunks.
+__global__ void chunk_mask_kernel(const DevTables T, DigestItem* __restrict__ items, const SubChunk* __restrict__ subs,
+                                  long long nitems, double tau, unsigned* __restrict__ mask)
+{
+    __shared__ int nnz;
+    for (long long ii = blockIdx.x; ii < nitems; ii += gridDim.x) {
+        const DigestItem it = items[ii];
+        const SubChunk sc = subs[it.sub];
+        const int I = sc.I, J = sc.J, view = it.view;
+        int R1, R2;
+        switch (view) {
+        case 0: R1 = I; R2 = J; break;
+        case 1: R1 = T.pair_I[it.a]; R2 = T.pair_J[it.a]; break;
+        case 2: R1 = I; R2 = it.a; break;
+        case 3: R1 = J; R2 = it.a; break;
+        case 4: R1 = I; R2 = it.a; break;
+        default: R1 = J; R2 = it.a; break;
+        }
+        const int nR2 = T.blk_nao[R2], nrows = T.blk_nao[R1] * nR2;
+        const int m0 = it.rowtile * kMT, m1 = min(m0 + kMT, nrows);
+        const int aoR1 = T.blk_ao0[R1], aoR2 = T.blk_ao0[R2];
+        if (threadIdx.x == 0) nnz = 0;
+        __syncthreads();
+        int mine = 0;
+        for (int q = threadIdx.x; q < it.nchunks; q += blockDim.x) {
+            // locate the step (panel) and the chunk inside it
+            int s = 0, ch = q, K = 0, L = 0, C1 = 0, C2 = 0;
+            for (; s < it.count; ++s) {
+                int rank;
+                step_blocks(T, it, s, K, L, rank);
+                switch (view) {
+                case 0: C1 = K; C2 = L; break;
+                case 1: C1 = I; C2 = J; break;
+                case 2: C1 = J; C2 = L; break;
+                case 3: C1 = I; C2 = L; break;
+                case 4: C1 = J; C2 = K; break;
+                default: C1 = I; C2 = K; break;
+                }
+                const int nch = (T.blk_nao[C1] * T.blk_nao[C2] + kKC - 1) / kKC;
+                if (ch < nch) break;
+                ch -= nch;
+            }
+            const int nC2 = T.blk_nao[C2], nC = T.blk_nao[C1] * nC2;
+            const int aoC1 = T.blk_ao0[C1], aoC2 = T.blk_ao0[C2];
+            const int c0 = ch * kKC, c1e = min(c0 + kKC, nC);
+            bool any = false;
+            int prev_cs1 = -1, prev_cs2 = -1;
+            for (int cidx = c0; cidx < c1e && !any; ++cidx) {
+                const int sc1 = T.ao_sh[aoC1 + cidx / nC2], sc2 = T.ao_sh[aoC2 + cidx % nC2];
+                if (sc1 == prev_cs1 && sc2 == prev_cs2) continue;       // same shell pair as the previous column
+                prev_cs1 = sc1; prev_cs2 = sc2;
+                int prev_rs1 = -1, prev_rs2 = -1;
+                for (int m = m0; m < m1; ++m) {
+                    const int sr1 = T.ao_sh[aoR1 + m / nR2], sr2 = T.ao_sh[aoR2 + m % nR2];
+                    if (sr1 == prev_rs1 && sr2 == prev_rs2) continue;
+                    prev_rs1 = sr1; prev_rs2 = sr2;
+                    int si, sj, sk, sl;
+                    switch (view) {
+                    case 0: si = sr1; sj = sr2; sk = sc1; sl = sc2; break;
+                    case 1: sk = sr1; sl = sr2; si = sc1; sj = sc2; break;
+                    case 2: si = sr1; sk = sr2; sj = sc1; sl = sc2; break;
+                    case 3: sj = sr1; sk = sr2; si = sc1; sl = sc2; break;
+                    case 4: si = sr1; sl = sr2; sj = sc1; sk = sc2; break;
+                    default: sj = sr1; sl = sr2; si = sc1; sk = sc2; break;
+                    }
+                    if (T.schwarz[(size_t)si * T.nshell + sj] * T.schwarz[(size_t)sk * T.nshell + sl] >= tau) { any = true; break; }
+                }
+            }
+            if (any) {
+                const unsigned bit = it.maskoff + (unsigned)q;
+                atomicOr(&mask[bit >> 5], 1u << (bit & 31u));
+                ++mine;
+            }
+        }
+        if (mine) atomicAdd(&nnz, mine);
+        __syncthreads();
+        if (threadIdx.x == 0) items[ii].nnz = nnz;
+        __syncthreads();
+    }
+}
+
+int launch_chunk_mask(ltjk_ctx* c)
+{
+    if (c->n_items == 0) return LTJK_OK;
+    LTJK_CUDA(c, cudaMemsetAsync(c->d_chunkmask, 0, sizeof(unsigned) * (size_t)(c->n_maskbits / 32 + 2), c->stream));
+    const int grid = (int)std::min<long long>(c->n_items, 148ll * 64);
+    chunk_mask_kernel<<<grid, 64, 0, c->stream>>>(c->t, c->d_items, c->d_subs, c->n_items, c->tau, c->d_chunkmask);
+    LTJK_CUDA(c, cudaGetLastError());
+    return LTJK_OK;
 }
 
 // ---------------------------------------------------------------------------------------------------------------

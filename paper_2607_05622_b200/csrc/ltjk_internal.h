@@ -30,6 +30,7 @@ struct DevTables {
     long long* koff = nullptr;     // [npair+1]  prefix sum of nao(I)*nao(J) over ranks
     int* rank_of = nullptr;        // [nblk*nblk] rank of block pair (I,J), I>=J (else -1)
     int* ao_perm = nullptr;        // [nao]      internal AO -> caller AO
+    int* ao_sh = nullptr;          // [nao]      internal AO -> internal shell
 };
 
 // A sub-chunk: the panels (IJ|KL) of one bra block pair and a run of ket ranks [r0,r1), contiguous in one half of
@@ -41,7 +42,7 @@ struct SubChunk {
     long long base;         // offset (doubles) of the first panel inside the ring half
 };
 
-// One digestion work item (24 bytes): a row tile of one output block accumulated over a run of panels.
+// One digestion work item (32 bytes): a row tile of one output block accumulated over a run of panels.
 struct DigestItem {
     unsigned char view;     // 0 JIJ, 1 JKL, 2 KIK, 3 KJK, 4 KIL, 5 KJL
     unsigned char partner;  // K views: 0 -> K[(r1,r2)] with D[(c1,c2)];  1 -> K[(r2,r1)] with D[(c2,c1)]
@@ -52,6 +53,8 @@ struct DigestItem {
     int count;              // panels in the run
     int sub;                // sub-chunk (global index)
     int nchunks;            // contraction chunks (of 16 columns) over the whole run: sum over panels of ceil(nC/16)
+    int nnz;                // chunks whose 128 x 16 tile holds at least one unscreened integral (set on the device)
+    unsigned maskoff;       // first bit of this item in the chunk mask
 };
 
 // A group: consecutive sub-chunks of one bra class that fit one ring half; one ERI launch per ket class and one
@@ -99,6 +102,8 @@ struct ltjk_ctx {
     ltjk::DevTables t;
     ltjk::DigestItem* d_items = nullptr;
     ltjk::SubChunk* d_subs = nullptr;
+    unsigned* d_chunkmask = nullptr;      // one bit per (item, chunk): tile not entirely screened
+    long long n_maskbits = 0;
     long long n_items = 0;
     double* d_panel = nullptr;            // integral panel staging ring (L2-sized)
     long long panel_cap = 0;              // doubles (both halves)
@@ -146,6 +151,7 @@ int launch_boys_debug(ltjk_ctx* c, int mmax, int n, const double* d_T, double* d
 
 // ltjk_digest.cu
 int launch_digest(ltjk_ctx* c, const Group& g, int nDp, bool doJ, bool doK);
+int launch_chunk_mask(ltjk_ctx* c);
 int launch_pack_densities(ltjk_ctx* c, int nD, int nDp, const double* D);
 int launch_unpack_results(ltjk_ctx* c, int nD, int nDp, double* J, double* K);
 int bench_dfma(ltjk_ctx* c, double* tflops);

@@ -213,3 +213,72 @@ def test_full_size_sweep_sampled_blocks(torch_cuda, name):
         ej = np.abs(Jh[:, x0:x1, y0:y1] - jb).reshape(len(ds), -1).max(1) / jmax
         ek = np.abs(Kh[:, x0:x1, y0:y1] - kb).reshape(len(ds), -1).max(1) / kmax
         assert ej.max() < TOL and ek.max() < TOL, ((X, Y), ej.max(), ek.max())
+
+
+def test_edge_cases_and_error_codes(torch_cuda, tiny):
+    """Degenerate inputs through the C ABI: call-order errors, l > 2, bad sizes, one density, a density count that
+    needs several column blocks (nD = 200 > 192), a one-shell basis (a single, fully diagonal block quartet)."""
+    torch = torch_cuda
+    from paper_2607_05622_b200 import ltjk
+    ctx = ltjk.Context(0)
+    D1 = torch.zeros((1, 4, 4), dtype=torch.float64, device="cuda")
+    with pytest.raises(ltjk.LtjkError) as e:
+        ctx.jk_build(D1, torch.empty_like(D1), torch.empty_like(D1))
+    assert e.value.code == -2                                     # LTJK_ENOBASIS
+    from paper_2607_05622_b200.inputs import Basis
+    bad = Basis(np.zeros((1, 3)), np.zeros(1, np.int32), np.array([3], np.int32), np.ones(1, np.int32),
+                np.zeros(1, np.int32), np.ones(1), np.ones(1), np.array([0, 10]))   # an f shell
+    with pytest.raises(ltjk.LtjkError) as e:
+        ctx.set_basis(bad)
+    assert e.value.code == -4                                     # LTJK_ELMAX
+    ctx.set_basis(tiny.basis)
+    with pytest.raises(ltjk.LtjkError) as e:
+        ctx.build_shell_pairs(-1.0)
+    assert e.value.code == -1                                     # LTJK_EINVAL
+    ctx.build_shell_pairs(tiny.schwarz_tau)
+    Dn = torch.zeros((1, tiny.nao, tiny.nao), dtype=torch.float64, device="cuda")
+    with pytest.raises(ltjk.LtjkError) as e:
+        ctx.jk_build(Dn, None, None)
+    assert e.value.code == -1
+    # zero density -> zero J, K (and finite)
+    J = torch.full_like(Dn, float("nan"))
+    K = torch.full_like(Dn, float("nan"))
+    ctx.jk_build(Dn, J, K)
+    torch.cuda.synchronize()
+    assert float(J.abs().max()) == 0.0 and float(K.abs().max()) == 0.0
+    # one density and 200 densities (two column blocks) agree with the oracle and with each other
+    D = random_densities(tiny.nao, 200, seed=21)
+    J200, K200 = gpu_jk(torch, ctx, D)
+    J1, K1 = gpu_jk(torch, ctx, D[137:138])
+    assert relerr(J1, J200[137:138]) < 1e-12 and relerr(K1, K200[137:138]) < 1e-12
+    Jr, Kr, _ = O.jk_folded(tiny.basis, D[[0, 137, 199]], tiny.schwarz_tau)
+    assert relerr(J200[[0, 137, 199]], Jr) < TOL and relerr(K200[[0, 137, 199]], Kr) < TOL
+    # linearity: K[sum c_d D_d] = sum c_d K[D_d]
+    cvec = np.random.default_rng(3).standard_normal(200)
+    Jc, Kc = gpu_jk(torch, ctx, np.tensordot(cvec, D, axes=1)[None])
+    assert relerr(Kc[0], np.tensordot(cvec, K200, axes=1)) < 1e-11
+    assert relerr(Jc[0], np.tensordot(cvec, J200, axes=1)) < 1e-11
+    # single d shell on one centre: one block, one fully diagonal block quartet (all three fold factors at once)
+    one = custom_basis(np.array([[0.3, -0.1, 0.2]]), [[(2, [0.9, 0.4], [0.6, 0.4])]])
+    c1 = make_ctx(one, tau=0.0)
+    Dd = random_densities(6, 2, seed=22)
+    Jg, Kg = gpu_jk(torch, c1, Dd)
+    Jd, Kd = O.jk_definition(O.eri_tensor(one), Dd)
+    assert relerr(Jg, Jd) < TOL and relerr(Kg, Kd) < TOL
+
+
+def test_symmetric_density_is_a_special_case(torch_cuda, small):
+    """the symmetric build is the A = B special case of the non-symmetric one; a symmetric-only
+    kernel would keep (K + K^T)/2 and silently drop the rest."""
+    w = small
+    D = random_densities(w.nao, 2, seed=31)
+    Ds = 0.5 * (D + D.transpose(0, 2, 1))
+    Da = 0.5 * (D - D.transpose(0, 2, 1))
+    ctx = make_ctx(w.basis)
+    J, K = gpu_jk(torch_cuda, ctx, D)
+    Js, Ks = gpu_jk(torch_cuda, ctx, Ds)
+    Ja, Ka = gpu_jk(torch_cuda, ctx, Da)
+    assert relerr(Ks, 0.5 * (K + K.transpose(0, 2, 1))) < 1e-11        # sym(K[D]) = K[sym D], and it is symmetric
+    assert relerr(Ka, 0.5 * (K - K.transpose(0, 2, 1))) < 1e-11        # antisym(K[D]) = K[antisym D] != 0
+    assert np.abs(Ka).max() > 1e-3 * np.abs(K).max()
+    assert relerr(Js, J) < 1e-11 and np.abs(Ja).max() < 1e-11 * np.abs(J).max()   # J only sees the symmetric part
