@@ -266,9 +266,15 @@ def main():
     digest_flops_alg = 20.0 * nD * ints                  # 2 J + 8 K FMAs per unique integral and density
     peak_tf = ctx.bench_dfma_peak()
     achieved_tf = digest_flops_alg / (st["digest_ms"] * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "digest_kernel (J/K digestion, all launches of one sweep)",
+    # DRAM traffic of the digestion launches of one sweep from the committed ncu capture (profiles/), 439 AO only
+    traffic = None
+    tfile = ROOT / "profiles" / "r1_digest_traffic.json"
+    if w.name == "porphine" and tfile.exists():
+        tj = json.loads(tfile.read_text())
+        traffic = tj["dram_bytes_read_per_sweep"] + tj["dram_bytes_write_per_sweep"]
+    roofline = {"bound": "alu", "kernel": "digest_kernel (J/K digestion; achieved = algorithmic flop of one sweep / summed duration of its launches)",
                 "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-                "traffic": None,
+                "traffic": traffic,
                 "peak_source": "DFMA microbenchmark in this run (ltjk_bench_dfma_peak); MEASURED_PEAKS.json has no fp64 entry",
                 "algorithmic_flops_per_sweep": digest_flops_alg, "executed_digest_flops_per_sweep": st["digest_flops"],
                 "digest_ms_per_sweep": st["digest_ms"], "eri_ms_per_sweep": st["eri_ms"],

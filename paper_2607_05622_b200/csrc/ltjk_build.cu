@@ -151,7 +151,7 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
         unsigned long long bits = 0;
         for (DigestItem& it : items) {
             if (bits + (unsigned long long)it.nchunks >= 0xffffffffull)
-                return set_err(c, LTJK_ENOMEM, "build_shell_pairs: chunk mask exceeds 2^32 bits");
+                return set_err(c, LTJK_ENOMEM, "build_shell_pairs: chunk mask exceeds 2^32 entries");
             it.maskoff = (unsigned)bits; it.nnz = it.nchunks;
             bits += (unsigned long long)it.nchunks;
         }
@@ -169,7 +169,7 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
         (rc = upload(c, &t.koff, c->koff)) || (rc = upload(c, &t.rank_of, c->rank_of)) ||
         (rc = upload(c, &t.ao_perm, c->ao_perm)) || (rc = upload(c, &t.ao_sh, ao_sh)))
         return rc;
-    LTJK_CUDA(c, cudaMalloc(&c->d_chunkmask, sizeof(unsigned) * (size_t)(c->n_maskbits / 32 + 2)));
+    LTJK_CUDA(c, cudaMalloc(&c->d_chunkmask, (size_t)c->n_maskbits + 16));
     if ((rc = launch_chunk_mask(c))) return rc;
     LTJK_CUDA(c, cudaStreamSynchronize(c->stream));
     c->have_pairs = true;

@@ -34,7 +34,7 @@ struct DigestArgs {
     const double* panel;
     const double* Dt;
     const double* Dst;
-    const unsigned* mask;
+    const unsigned char* mask;   // per (item, chunk): bit w set = the 16 x 16 sub-tile of consumer warp w is not all screened
     double* Jt;
     double* Kt;
     int nDp;
@@ -87,6 +87,7 @@ struct DigestSmem {
     double B[kStages][kKC][32 * TN];
     unsigned long long full[kStages];    // producer -> consumers: the stage's tiles have landed
     unsigned long long empty[kStages];   // consumers -> producer: the stage may be refilled
+    unsigned cmask[kStages];             // warp bits of the chunk in the stage (written by producer thread 0)
     int rowoff[kMT];
     int acol[kMaxNC];
     unsigned bcol[kMaxNC];
@@ -152,7 +153,7 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
 
     if (tid == 0) {
         for (int st = 0; st < kStages; ++st) {
-            mbar_init(&S.full[st], kProducerThreads);
+            mbar_init(&S.full[st], kProducerThreads + 1);   // 128 cp.async arrivals + the thread that posts cmask
             mbar_init(&S.empty[st], kConsumerWarps);
         }
     }
@@ -203,8 +204,8 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
                 const int ro_fixed = S.rowoff[pt];                            // rowContig: this thread's row
                 for (int ch = 0; ch < nch; ++ch, ++qi) {
                     // tiles whose integrals are all Schwarz-screened (exact zeros in the panel) are never loaded
-                    const unsigned bit = it.maskoff + (unsigned)qi;
-                    if (!((g.mask[bit >> 5] >> (bit & 31u)) & 1u)) continue;
+                    const unsigned wbits = g.mask[(size_t)it.maskoff + (unsigned)qi];
+                    if (!wbits) continue;
                     const int st = gch % kStages;
                     if (gch >= kStages) mbar_wait(&S.empty[st], (unsigned)((gch / kStages - 1) & 1));
                     // A tile: kKC x kMT elements of 8 bytes, 16 per producer thread, lanes along the unit stride
@@ -236,6 +237,7 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
                             cp_async16(&S.B[st][k][pc * 2], src + (ok ? pc * 2 : 0), ok);
                     }
                     mbar_arrive_on_cp_async(&S.full[st]);
+                    if (pt == 0) { S.cmask[st] = wbits; mbar_arrive(&S.full[st]); }   // release: visible after the wait
                     ++gch;
                 }
             }
@@ -261,7 +263,7 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
         for (int q = 0; q < total_chunks; ++q, ++gch) {
             const int st = gch % kStages;
             mbar_wait(&S.full[st], (unsigned)((gch / kStages) & 1));
-            if (warp_active) {
+            if (warp_active && ((S.cmask[st] >> w) & 1u)) {
 #pragma unroll
                 for (int k = 0; k < kKC; ++k) {
                     const double2* ap = reinterpret_cast<const double2*>(&S.A[st][k][trow]);
@@ -361,7 +363,7 @@ int launch_digest(ltjk_ctx* c, const Group& ch, int nDp, bool doJ, bool doK)
 // a5, geometry-frozen: for every work item and every contraction chunk, does the 128 x 16 tile of the panel view hold
 // at least one integral of an unscreened shell quartet (Q_ij Q_kl >= tau)?  One CTA per item, threads over chunks.
 __global__ void chunk_mask_kernel(const DevTables T, DigestItem* __restrict__ items, const SubChunk* __restrict__ subs,
-                                  long long nitems, double tau, unsigned* __restrict__ mask)
+                                  long long nitems, double tau, unsigned char* __restrict__ mask)
 {
     __shared__ int nnz;
     for (long long ii = blockIdx.x; ii < nitems; ii += gridDim.x) {
@@ -404,14 +406,17 @@ __global__ void chunk_mask_kernel(const DevTables T, DigestItem* __restrict__ it
             const int nC2 = T.blk_nao[C2], nC = T.blk_nao[C1] * nC2;
             const int aoC1 = T.blk_ao0[C1], aoC2 = T.blk_ao0[C2];
             const int c0 = ch * kKC, c1e = min(c0 + kKC, nC);
+            unsigned wbits = 0;
+            for (int wq = 0; wq < kConsumerWarps; ++wq) {
+            const int mw0 = m0 + wq * kTM, mw1 = min(mw0 + kTM, m1);
             bool any = false;
             int prev_cs1 = -1, prev_cs2 = -1;
-            for (int cidx = c0; cidx < c1e && !any; ++cidx) {
+            for (int cidx = c0; cidx < c1e && !any && mw0 < mw1; ++cidx) {
                 const int sc1 = T.ao_sh[aoC1 + cidx / nC2], sc2 = T.ao_sh[aoC2 + cidx % nC2];
                 if (sc1 == prev_cs1 && sc2 == prev_cs2) continue;       // same shell pair as the previous column
                 prev_cs1 = sc1; prev_cs2 = sc2;
                 int prev_rs1 = -1, prev_rs2 = -1;
-                for (int m = m0; m < m1; ++m) {
+                for (int m = mw0; m < mw1; ++m) {
                     const int sr1 = T.ao_sh[aoR1 + m / nR2], sr2 = T.ao_sh[aoR2 + m % nR2];
                     if (sr1 == prev_rs1 && sr2 == prev_rs2) continue;
                     prev_rs1 = sr1; prev_rs2 = sr2;
@@ -427,11 +432,10 @@ __global__ void chunk_mask_kernel(const DevTables T, DigestItem* __restrict__ it
                     if (T.schwarz[(size_t)si * T.nshell + sj] * T.schwarz[(size_t)sk * T.nshell + sl] >= tau) { any = true; break; }
                 }
             }
-            if (any) {
-                const unsigned bit = it.maskoff + (unsigned)q;
-                atomicOr(&mask[bit >> 5], 1u << (bit & 31u));
-                ++mine;
+            if (any) wbits |= 1u << wq;
             }
+            mask[(size_t)it.maskoff + (unsigned)q] = (unsigned char)wbits;
+            if (wbits) ++mine;
         }
         if (mine) atomicAdd(&nnz, mine);
         __syncthreads();
@@ -443,7 +447,6 @@ __global__ void chunk_mask_kernel(const DevTables T, DigestItem* __restrict__ it
 int launch_chunk_mask(ltjk_ctx* c)
 {
     if (c->n_items == 0) return LTJK_OK;
-    LTJK_CUDA(c, cudaMemsetAsync(c->d_chunkmask, 0, sizeof(unsigned) * (size_t)(c->n_maskbits / 32 + 2), c->stream));
     const int grid = (int)std::min<long long>(c->n_items, 148ll * 64);
     chunk_mask_kernel<<<grid, 64, 0, c->stream>>>(c->t, c->d_items, c->d_subs, c->n_items, c->tau, c->d_chunkmask);
     LTJK_CUDA(c, cudaGetLastError());

@@ -54,7 +54,7 @@ struct DigestItem {
     int sub;                // sub-chunk (global index)
     int nchunks;            // contraction chunks (of 16 columns) over the whole run: sum over panels of ceil(nC/16)
     int nnz;                // chunks whose 128 x 16 tile holds at least one unscreened integral (set on the device)
-    unsigned maskoff;       // first bit of this item in the chunk mask
+    unsigned maskoff;       // first byte of this item in the chunk mask
 };
 
 // A group: consecutive sub-chunks of one bra class that fit one ring half; one ERI launch per ket class and one
@@ -102,7 +102,7 @@ struct ltjk_ctx {
     ltjk::DevTables t;
     ltjk::DigestItem* d_items = nullptr;
     ltjk::SubChunk* d_subs = nullptr;
-    unsigned* d_chunkmask = nullptr;      // one bit per (item, chunk): tile not entirely screened
+    unsigned char* d_chunkmask = nullptr; // one byte per (item, chunk): bit w = sub-tile of consumer warp w not entirely screened
     long long n_maskbits = 0;
     long long n_items = 0;
     double* d_panel = nullptr;            // integral panel staging ring (L2-sized)
