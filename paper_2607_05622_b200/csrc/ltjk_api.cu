@@ -18,7 +18,9 @@ int set_err(ltjk_ctx* c, int code, const std::string& msg)
 
 void digest_colblocks(int nD, int* TN, int* ncolblk);   // ltjk_digest.cu
 
-static const int kBlkShells[3] = {16, 5, 3};   // target shells per block for l = 0,1,2 (16 / 15 / 18 AOs)
+// Shells per block for l = 0,1,2: 16 / 24 / 24 AOs.  Output blocks of the digestion then have 256, 384 or 576 rows
+// = 2, 3 or 4.5 row tiles of 128: measured tile fill 94 % against 82 % with the first choice (16/15/18, split evenly).
+static const int kBlkShells[3] = {16, 8, 4};
 static const int kRunMax = 8;                  // panels accumulated in registers before a flush
 
 template <class T>
@@ -340,7 +342,7 @@ int ltjk_set_basis(ltjk_ctx* c, int natom, const double* xyz, int nshell, const 
         c->sh_ao_int[s] = ao;
         for (int k = 0; k < ncart(l[e]); ++k) c->ao_perm[ao++] = ao_ext[e] + k;
     }
-    // l-homogeneous blocks, evenly split
+    // l-homogeneous blocks of fixed size (the last one of each l takes the remainder)
     c->blk_sh0.clear(); c->blk_nsh.clear(); c->blk_ao0.clear(); c->blk_nao.clear(); c->blk_l.clear();
     int s0 = 0;
     for (int ll = 0; ll < 3; ++ll) {
@@ -351,7 +353,7 @@ int ltjk_set_basis(ltjk_ctx* c, int natom, const double* xyz, int nshell, const 
         const int nb = (n + kBlkShells[ll] - 1) / kBlkShells[ll];
         int done = 0;
         for (int b = 0; b < nb; ++b) {
-            const int cnt = (n - done + (nb - b) - 1) / (nb - b);
+            const int cnt = std::min(kBlkShells[ll], n - done);   // full blocks, then one remainder block
             c->blk_sh0.push_back(s0 + done); c->blk_nsh.push_back(cnt);
             c->blk_ao0.push_back(c->sh_ao_int[s0 + done]); c->blk_nao.push_back(cnt * ncart(ll));
             c->blk_l.push_back(ll);
