@@ -109,6 +109,19 @@ int ltjk_sweep_host(ltjk_ctx* ctx, int nocc, int nvir, const double* C_occ_host,
                     const double* eps_occ_host, const double* eps_vir_host, int nT, const double* T_host, int ntau,
                     const double* tau_host, double* J_host, double* K_host);
 
+/* Laplace-Fock back-transform (Eq. 19), per density d:
+ *   F[d][p][q] = sum_{mu nu} C[mu][p] (2 J[d] - K[d])[mu][nu] C[nu][q]
+ * DEVICE pointers, row-major: J, K [nD][N][N], C [N][nmo], F [nD][nmo][nmo] (overwritten).  Two batched fp64
+ * tensor-core GEMMs; enqueued on the context stream. */
+int ltjk_laplace_fock(ltjk_ctx* ctx, int nD, const double* J, const double* K, int nmo, const double* C, double* F);
+
+/* Quadrature-weighted accumulation over the Laplace grid with the EOM reweighting (Eq. 11, L180 Eq. 21):
+ *   Y[t][e] = sum_a w[a] exp(omega tau[a]) X[a][t][e],   e < nelem
+ * X [ntau][nT][nelem], Y [nT][nelem] DEVICE pointers; tau_host, w_host HOST arrays [ntau]; omega = 0 gives the plain
+ * weights.  The caller is responsible for omega < min denominator (Eq. 21's validity range). */
+int ltjk_laplace_accumulate(ltjk_ctx* ctx, int ntau, int nT, long long nelem, const double* tau_host,
+                            const double* w_host, double omega, const double* X, double* Y);
+
 /* Statistics of the last ltjk_jk_build on this context (HOST outputs, any may be NULL):
  *   n_launches    kernels launched
  *   eri_quartets  contracted shell quartets evaluated (4-fold unique: A>=B, C>=D, all bra x ket)

@@ -295,3 +295,35 @@ def laplace_minimax(xmin: float, xmax: float, k: int, verbose: bool = False):
 def laplace_error_curve(tau, w, x):
     x = np.asarray(x, dtype=np.float64)
     return 1.0 / x - (np.asarray(w)[None, :] * np.exp(-x[:, None] * np.asarray(tau)[None, :])).sum(1)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# SURVEY 8(f) N1.  Laplace-Fock back-transform, Eq. (19):
+#     F~[d]_pq = sum_{mu nu} C_{mu p} (2 J[d] - K[d])_{mu nu} C_{nu q}
+# written as the definition (an einsum, a library contraction as the step), and the quadrature-weighted grid sum with
+# the EOM reweighting, Eqs. (11), (21):  Y[t] = sum_a w_a exp(omega tau_a) X[a][t].
+def laplace_fock(J: np.ndarray, K: np.ndarray, C: np.ndarray) -> np.ndarray:
+    return np.einsum("mp,dmn,nq->dpq", C, 2.0 * J - K, C, optimize=True)
+
+
+def laplace_fock_loops(J: np.ndarray, K: np.ndarray, C: np.ndarray) -> np.ndarray:
+    """Eq. (19) as explicit loops (small cases; pins the einsum)."""
+    nD, n, _ = J.shape
+    nmo = C.shape[1]
+    F = np.zeros((nD, nmo, nmo))
+    for d in range(nD):
+        for p in range(nmo):
+            for q in range(nmo):
+                s = 0.0
+                for mu in range(n):
+                    for nu in range(n):
+                        s += C[mu, p] * (2.0 * J[d, mu, nu] - K[d, mu, nu]) * C[nu, q]
+                F[d, p, q] = s
+    return F
+
+
+def laplace_accumulate(tau, w, omega: float, X: np.ndarray) -> np.ndarray:
+    out = np.zeros(X.shape[1:])
+    for a in range(X.shape[0]):
+        out += w[a] * np.exp(omega * tau[a]) * X[a]        # w~_a(omega) = w_a e^{omega tau_a}, Eq. (21)
+    return out

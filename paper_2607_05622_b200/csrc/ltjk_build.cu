@@ -325,6 +325,25 @@ int ltjk_sweep_host(ltjk_ctx* c, int nocc, int nvir, const double* C_occ_host, c
     return LTJK_OK;
 }
 
+int ltjk_laplace_fock(ltjk_ctx* c, int nD, const double* J, const double* K, int nmo, const double* C, double* F)
+{
+    if (!c) return LTJK_EINVAL;
+    if (!c->have_basis) return set_err(c, LTJK_ENOBASIS, "laplace_fock: no basis");
+    if (nD <= 0 || nmo <= 0 || !J || !K || !C || !F) return set_err(c, LTJK_EINVAL, "laplace_fock: bad arguments");
+    cudaSetDevice(c->device);
+    return launch_laplace_fock(c, nD, J, K, nmo, C, F);
+}
+
+int ltjk_laplace_accumulate(ltjk_ctx* c, int ntau, int nT, long long nelem, const double* tau_host,
+                            const double* w_host, double omega, const double* X, double* Y)
+{
+    if (!c) return LTJK_EINVAL;
+    if (ntau <= 0 || nT <= 0 || nelem <= 0 || !tau_host || !w_host || !X || !Y)
+        return set_err(c, LTJK_EINVAL, "laplace_accumulate: bad arguments");
+    cudaSetDevice(c->device);
+    return launch_laplace_accumulate(c, ntau, nT, nelem, tau_host, w_host, omega, X, Y);
+}
+
 int ltjk_get_stats(const ltjk_ctx* c, long long* n_launches, long long* eri_quartets, double* digest_flops,
                    double* eri_ms, double* digest_ms)
 {

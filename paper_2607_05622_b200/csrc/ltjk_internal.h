@@ -162,4 +162,8 @@ int launch_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C_occ
                             const double* eps_occ, const double* eps_vir, int nT, const double* T, int ntau,
                             const double* tau_host, double* D_out);
 
+int launch_laplace_fock(ltjk_ctx* c, int nD, const double* J, const double* K, int nmo, const double* C, double* F);
+int launch_laplace_accumulate(ltjk_ctx* c, int ntau, int nT, long long nelem, const double* tau_host,
+                              const double* w_host, double omega, const double* X, double* Y);
+
 }  // namespace ltjk

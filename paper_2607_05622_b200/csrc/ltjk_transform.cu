@@ -5,6 +5,8 @@
 //   D = C_o . W                                          (N x N)
 // (nocc < nvir, so contracting the virtual index first is the cheaper order.)
 #include "ltjk_internal.h"
+#include <algorithm>
+#include <cmath>
 
 namespace ltjk {
 
@@ -29,6 +31,7 @@ struct GemmArgs {
     const double* A; long long sAa, sAb;
     const double* B; long long sBa, sBb;
     double* C; long long sCa, sCb;
+    const double* A2; double ca, ca2;    // optional second A operand: A_eff = ca * A + ca2 * A2 (same strides)
     const double* sr; long long ssr;     // row scale, per za (may be null)
     const double* sc; long long ssc;     // column (k) scale, per za
     int nzb;
@@ -54,6 +57,7 @@ __global__ void __launch_bounds__(256) gemm_kernel(const GemmArgs g)
     __shared__ double Bs[BK][LD];
     const int za = blockIdx.z / g.nzb, zb = blockIdx.z % g.nzb;
     const double* __restrict__ A = g.A + za * g.sAa + zb * g.sAb;
+    const double* __restrict__ A2 = g.A2 ? g.A2 + za * g.sAa + zb * g.sAb : nullptr;
     const double* __restrict__ B = g.B + za * g.sBa + zb * g.sBb;
     double* __restrict__ C = g.C + za * g.sCa + zb * g.sCb;
     const double* sr = g.sr ? g.sr + za * g.ssr : nullptr;
@@ -72,6 +76,7 @@ __global__ void __launch_bounds__(256) gemm_kernel(const GemmArgs g)
             double v = 0.0;
             if (gm < g.M && gk < g.K) {
                 v = A[(size_t)gm * g.K + gk];
+                if (A2) v = g.ca * v + g.ca2 * A2[(size_t)gm * g.K + gk];
                 if (sr) v *= sr[gm] * sc[gk];
             }
             As[k][m] = v;
@@ -138,7 +143,7 @@ int launch_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C_occ
     g1.A = T; g1.sAa = 0; g1.sAb = (long long)nocc * nvir;
     g1.B = C_vir; g1.sBa = 0; g1.sBb = 0;
     g1.C = W; g1.sCa = (long long)nT * nocc * N; g1.sCb = (long long)nocc * N;
-    g1.sr = fo; g1.ssr = nocc; g1.sc = fv; g1.ssc = nvir; g1.nzb = nT;
+    g1.sr = fo; g1.ssr = nocc; g1.sc = fv; g1.ssc = nvir; g1.nzb = nT; g1.A2 = nullptr; g1.ca = 1.0; g1.ca2 = 0.0;
     gemm_kernel<true><<<dim3((N + 63) / 64, (nocc + 63) / 64, ntau * nT), 256, 0, c->stream>>>(g1);
     LTJK_CUDA(c, cudaGetLastError());
     GemmArgs g2;   // D[a][d] = C_occ . W[a][d]
@@ -146,11 +151,81 @@ int launch_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C_occ
     g2.A = C_occ; g2.sAa = 0; g2.sAb = 0;
     g2.B = W; g2.sBa = (long long)nT * nocc * N; g2.sBb = (long long)nocc * N;
     g2.C = D_out; g2.sCa = (long long)nT * N * N; g2.sCb = (long long)N * N;
-    g2.sr = nullptr; g2.ssr = 0; g2.sc = nullptr; g2.ssc = 0; g2.nzb = nT;
+    g2.sr = nullptr; g2.ssr = 0; g2.sc = nullptr; g2.ssc = 0; g2.nzb = nT; g2.A2 = nullptr; g2.ca = 1.0; g2.ca2 = 0.0;
     gemm_kernel<false><<<dim3((N + 63) / 64, (N + 63) / 64, ntau * nT), 256, 0, c->stream>>>(g2);
     LTJK_CUDA(c, cudaGetLastError());
     cudaFreeAsync(tau, c->stream); cudaFreeAsync(fo, c->stream); cudaFreeAsync(fv, c->stream); cudaFreeAsync(W, c->stream);
     c->st_launches += 3;
+    return LTJK_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------
+// Laplace-Fock back-transform (Eq. 19) and grid accumulation (Eqs. 11, 21).
+__global__ void transpose_kernel(int rows, int cols, const double* __restrict__ in, double* __restrict__ out)
+{
+    __shared__ double tile[32][33];
+    const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
+    for (int i = threadIdx.y; i < 32; i += 8)
+        if (r0 + i < rows && c0 + threadIdx.x < cols) tile[i][threadIdx.x] = in[(size_t)(r0 + i) * cols + c0 + threadIdx.x];
+    __syncthreads();
+    for (int i = threadIdx.y; i < 32; i += 8)
+        if (c0 + i < cols && r0 + threadIdx.x < rows) out[(size_t)(c0 + i) * rows + r0 + threadIdx.x] = tile[threadIdx.x][i];
+}
+
+int launch_laplace_fock(ltjk_ctx* c, int nD, const double* J, const double* K, int nmo, const double* C, double* F)
+{
+    const int N = c->nao;
+    double *Ct = nullptr, *tmp = nullptr;
+    LTJK_CUDA(c, cudaMallocAsync(&Ct, sizeof(double) * (size_t)N * nmo, c->stream));
+    LTJK_CUDA(c, cudaMallocAsync(&tmp, sizeof(double) * (size_t)nD * N * nmo, c->stream));
+    transpose_kernel<<<dim3((nmo + 31) / 32, (N + 31) / 32), dim3(32, 8), 0, c->stream>>>(N, nmo, C, Ct);
+    LTJK_CUDA(c, cudaGetLastError());
+    GemmArgs g1;   // tmp[d] (N x nmo) = (2 J[d] - K[d]) . C
+    g1.M = N; g1.Nn = nmo; g1.K = N;
+    g1.A = J; g1.A2 = K; g1.ca = 2.0; g1.ca2 = -1.0; g1.sAa = (long long)N * N; g1.sAb = 0;
+    g1.B = C; g1.sBa = 0; g1.sBb = 0;
+    g1.C = tmp; g1.sCa = (long long)N * nmo; g1.sCb = 0;
+    g1.sr = nullptr; g1.ssr = 0; g1.sc = nullptr; g1.ssc = 0; g1.nzb = 1;
+    gemm_kernel<false><<<dim3((nmo + 63) / 64, (N + 63) / 64, nD), 256, 0, c->stream>>>(g1);
+    LTJK_CUDA(c, cudaGetLastError());
+    GemmArgs g2;   // F[d] (nmo x nmo) = C^T . tmp[d]
+    g2.M = nmo; g2.Nn = nmo; g2.K = N;
+    g2.A = Ct; g2.A2 = nullptr; g2.ca = 1.0; g2.ca2 = 0.0; g2.sAa = 0; g2.sAb = 0;
+    g2.B = tmp; g2.sBa = (long long)N * nmo; g2.sBb = 0;
+    g2.C = F; g2.sCa = (long long)nmo * nmo; g2.sCb = 0;
+    g2.sr = nullptr; g2.ssr = 0; g2.sc = nullptr; g2.ssc = 0; g2.nzb = 1;
+    gemm_kernel<false><<<dim3((nmo + 63) / 64, (nmo + 63) / 64, nD), 256, 0, c->stream>>>(g2);
+    LTJK_CUDA(c, cudaGetLastError());
+    cudaFreeAsync(Ct, c->stream); cudaFreeAsync(tmp, c->stream);
+    return LTJK_OK;
+}
+
+__global__ void accumulate_kernel(int ntau, int nT, long long nelem, const double* __restrict__ wt,
+                                  const double* __restrict__ X, double* __restrict__ Y)
+{
+    const long long tot = (long long)nT * nelem;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < tot; i += (long long)gridDim.x * blockDim.x) {
+        double s = 0.0;
+        for (int a = 0; a < ntau; ++a) s = fma(wt[a], X[(size_t)a * tot + i], s);
+        Y[i] = s;
+    }
+}
+
+int launch_laplace_accumulate(ltjk_ctx* c, int ntau, int nT, long long nelem, const double* tau_host,
+                              const double* w_host, double omega, const double* X, double* Y)
+{
+    std::vector<double> wt(ntau);
+    for (int a = 0; a < ntau; ++a) wt[a] = w_host[a] * exp(omega * tau_host[a]);   // Eq. 21
+    double* d_w = nullptr;
+    LTJK_CUDA(c, cudaMallocAsync(&d_w, sizeof(double) * ntau, c->stream));
+    LTJK_CUDA(c, cudaMemcpyAsync(d_w, wt.data(), sizeof(double) * ntau, cudaMemcpyHostToDevice, c->stream));
+    LTJK_CUDA(c, cudaStreamSynchronize(c->stream));      // wt is a local buffer
+    const long long tot = (long long)nT * nelem;
+    const int grid = (int)std::min<long long>((tot + 255) / 256, 148ll * 16);
+    accumulate_kernel<<<grid, 256, 0, c->stream>>>(ntau, nT, nelem, d_w, X, Y);
+    LTJK_CUDA(c, cudaGetLastError());
+    cudaFreeAsync(d_w, c->stream);
     return LTJK_OK;
 }
 

@@ -23,7 +23,7 @@ ERRORS = {0: "LTJK_OK", -1: "LTJK_EINVAL", -2: "LTJK_ENOBASIS", -3: "LTJK_ECUDA"
 EXPORTS = [
     "ltjk_create", "ltjk_destroy", "ltjk_last_error", "ltjk_set_scratch_bytes", "ltjk_set_basis", "ltjk_get_nao",
     "ltjk_build_shell_pairs", "ltjk_get_schwarz", "ltjk_laplace_quadrature", "ltjk_build_pseudo_densities",
-    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_get_stats", "ltjk_set_timing", "ltjk_debug_eri_quartet",
+    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_laplace_fock", "ltjk_laplace_accumulate", "ltjk_get_stats", "ltjk_set_timing", "ltjk_debug_eri_quartet",
     "ltjk_debug_boys", "ltjk_bench_dfma_peak", "ltjk_bench_copy_peak",
 ]
 
@@ -193,6 +193,22 @@ class Context:
         self._chk(self.lib.ltjk_sweep_host(
             self._h, ctypes.c_int(C_occ.shape[1]), ctypes.c_int(C_vir.shape[1]), hp(C_occ), hp(C_vir), hp(eps_occ),
             hp(eps_vir), ctypes.c_int(T.shape[0]), hp(T), ctypes.c_int(tau.shape[0]), _d(tau), hp(J), hp(K)))
+
+    def laplace_fock(self, J, K, C, F):
+        """ltjk_laplace_fock: F[d] = C^T (2 J[d] - K[d]) C; device tensors J, K [nD,N,N], C [N,nmo], F [nD,nmo,nmo]."""
+        self._chk(self.lib.ltjk_laplace_fock(self._h, ctypes.c_int(J.shape[0]), _devptr(J), _devptr(K),
+                                             ctypes.c_int(C.shape[1]), _devptr(C), _devptr(F)))
+
+    def laplace_accumulate(self, tau, w, omega, X, Y):
+        """ltjk_laplace_accumulate: Y[t] = sum_a w_a exp(omega tau_a) X[a][t]; X [ntau,nT,...], Y [nT,...] device."""
+        tau = np.ascontiguousarray(tau, dtype=np.float64)
+        w = np.ascontiguousarray(w, dtype=np.float64)
+        nelem = 1
+        for n in Y.shape[1:]:
+            nelem *= int(n)
+        self._chk(self.lib.ltjk_laplace_accumulate(self._h, ctypes.c_int(X.shape[0]), ctypes.c_int(X.shape[1]),
+                                                   ctypes.c_longlong(nelem), _d(tau), _d(w), ctypes.c_double(omega),
+                                                   _devptr(X), _devptr(Y)))
 
     def get_stats(self) -> dict:
         nl = ctypes.c_longlong(0)

@@ -282,3 +282,53 @@ def test_symmetric_density_is_a_special_case(torch_cuda, small):
     assert relerr(Ka, 0.5 * (K - K.transpose(0, 2, 1))) < 1e-11        # antisym(K[D]) = K[antisym D] != 0
     assert np.abs(Ka).max() > 1e-3 * np.abs(K).max()
     assert relerr(Js, J) < 1e-11 and np.abs(Ja).max() < 1e-11 * np.abs(J).max()   # J only sees the symmetric part
+
+
+def test_laplace_cascade_closure(torch_cuda, small):
+    """The path's purpose end to end: library grid -> pseudo-densities -> J/K -> weighted
+    accumulation resolves the orbital-energy denominator,
+        sum_a w_a K[D^a] = K[C_o (T o 1/(eps_v - eps_o)) C_v^T]      (same for J)
+    to the quadrature error, and the Laplace-Fock back-transform (Eq. 19) matches the oracle."""
+    torch = torch_cuda
+    from paper_2607_05622_b200 import ltjk
+    w = small
+    N = w.nao
+    tau, wts, err = ltjk.laplace_quadrature(w.laplace_range[0], w.laplace_range[1], w.ntau)
+    ctx = make_ctx(w.basis)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    D = torch.empty((w.ntau, w.nT, N, N), dtype=torch.float64, device="cuda")
+    ctx.build_pseudo_densities(dev(w.C_occ), dev(w.C_vir), dev(w.eps_occ), dev(w.eps_vir), dev(w.T), tau, D)
+    Dn = D.view(-1, N, N)
+    J = torch.empty_like(Dn)
+    K = torch.empty_like(Dn)
+    ctx.jk_build(Dn, J, K)
+    Ksum = torch.empty((w.nT, N, N), dtype=torch.float64, device="cuda")
+    Jsum = torch.empty_like(Ksum)
+    ctx.laplace_accumulate(tau, wts, 0.0, K.view(w.ntau, w.nT, N, N), Ksum)
+    ctx.laplace_accumulate(tau, wts, 0.0, J.view(w.ntau, w.nT, N, N), Jsum)
+    # exact denominators on the GPU path too (one build per amplitude set)
+    denom = w.eps_vir[None, :] - w.eps_occ[:, None]
+    assert denom.min() >= w.laplace_range[0] and denom.max() <= w.laplace_range[1]
+    Dex = np.einsum("mi,tia,na->tmn", w.C_occ, w.T / denom[None], w.C_vir)
+    Jex, Kex = gpu_jk(torch, ctx, Dex)
+    scale = np.abs(np.einsum("mi,tia,na->tmn", np.abs(w.C_occ), np.abs(w.T), np.abs(w.C_vir))).max()
+    tol = 50 * err * scale * np.abs(Kex).max() / np.abs(Dex).max()
+    assert np.abs(Ksum.cpu().numpy() - Kex).max() < tol and np.abs(Jsum.cpu().numpy() - Jex).max() < tol * 10
+    assert relerr(Ksum.cpu().numpy(), Kex) < 1e-6 and relerr(Jsum.cpu().numpy(), Jex) < 1e-6
+    # accumulation itself: oracle parity at 1e-13, including the omega reweighting of Eq. 21
+    Kh = K.cpu().numpy().reshape(w.ntau, w.nT, N, N)
+    assert relerr(Ksum.cpu().numpy(), O.laplace_accumulate(tau, wts, 0.0, Kh)) < 1e-13
+    ctx.laplace_accumulate(tau, wts, 0.2, K.view(w.ntau, w.nT, N, N), Ksum)
+    assert relerr(Ksum.cpu().numpy(), O.laplace_accumulate(tau, wts, 0.2, Kh)) < 1e-13
+    # Laplace-Fock back-transform on a few densities
+    C = np.ascontiguousarray(np.concatenate([w.C_occ, w.C_vir], axis=1))
+    F = torch.empty((4, N, N), dtype=torch.float64, device="cuda")
+    ctx.laplace_fock(J[:4].contiguous(), K[:4].contiguous(), dev(C), F)
+    torch.cuda.synchronize()
+    Fr = O.laplace_fock(J[:4].cpu().numpy(), K[:4].cpu().numpy(), C)
+    assert relerr(F.cpu().numpy(), Fr) < 1e-12
+    # rectangular MO block (occupied columns only)
+    Fo = torch.empty((4, w.nocc, w.nocc), dtype=torch.float64, device="cuda")
+    ctx.laplace_fock(J[:4].contiguous(), K[:4].contiguous(), dev(w.C_occ), Fo)
+    torch.cuda.synchronize()
+    assert relerr(Fo.cpu().numpy(), Fr[:, :w.nocc, :w.nocc]) < 1e-12
