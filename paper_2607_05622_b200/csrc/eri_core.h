@@ -149,9 +149,11 @@ LTJK_HD void eri_quartet(const double* __restrict__ bra, const double* __restric
         for (int jf = 0; jf < NF; ++jf) HB::run(acc + jf, NF, out + jf, NF, bra[0], bra[1], bra[2]);
         return;
     }
-    double t1[NAB * NF];
-    for (int jf = 0; jf < NF; ++jf) HB::run(acc + jf, NF, t1 + jf, NF, bra[0], bra[1], bra[2]);
-    for (int iab = 0; iab < NAB; ++iab) HK::run(t1 + iab * NF, 1, out + iab * NCD, 1, ket[0], ket[1], ket[2]);
+    if (LB > 0 && LD > 0) {
+        double t1[NAB * NF];
+        for (int jf = 0; jf < NF; ++jf) HB::run(acc + jf, NF, t1 + jf, NF, bra[0], bra[1], bra[2]);
+        for (int iab = 0; iab < NAB; ++iab) HK::run(t1 + iab * NF, 1, out + iab * NCD, 1, ket[0], ket[1], ket[2]);
+    }
 }
 
 }  // namespace ltjk

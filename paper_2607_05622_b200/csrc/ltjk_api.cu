@@ -16,22 +16,10 @@ int set_err(ltjk_ctx* c, int code, const std::string& msg)
     return code;
 }
 
-void digest_colblocks(int nD, int* TN, int* ncolblk);   // ltjk_digest.cu
-
 // Shells per block for l = 0,1,2: 16 / 24 / 24 AOs.  Output blocks of the digestion then have 256, 384 or 576 rows
 // = 2, 3 or 4.5 row tiles of 128: measured tile fill 94 % against 82 % with the first choice (16/15/18, split evenly).
 static const int kBlkShells[3] = {16, 8, 4};
 static const int kRunMax = 8;                  // panels accumulated in registers before a flush
-
-template <class T>
-int upload_impl(ltjk_ctx* c, T** dst, const std::vector<T>& src)
-{
-    if (*dst) { cudaFree(*dst); *dst = nullptr; }
-    if (src.empty()) return LTJK_OK;
-    LTJK_CUDA(c, cudaMalloc((void**)dst, sizeof(T) * src.size()));
-    LTJK_CUDA(c, cudaMemcpyAsync(*dst, src.data(), sizeof(T) * src.size(), cudaMemcpyHostToDevice, c->stream));
-    return LTJK_OK;
-}
 
 void free_tables(ltjk_ctx* c)
 {
@@ -78,7 +66,6 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
     Group g;
     bool open = false;
     long long used = 0;                                   // doubles used in the current ring half
-    size_t j_first = 0;
     std::vector<DigestItem> jitems, kitems;
     // contraction chunks of an item (the consumers of the digestion kernel need the count up front)
     auto fill_chunks = [&](DigestItem& it) {
@@ -120,7 +107,6 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
         c->groups.push_back(g);
         open = false;
     };
-    (void)j_first;
     for (int rIJ = 0; rIJ < npair; ++rIJ) {
         const int I = c->pair_I[rIJ], J = c->pair_J[rIJ];
         const int nI = c->blk_nao[I], nJ = c->blk_nao[J];
