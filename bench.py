@@ -261,6 +261,17 @@ def main():
     torch.cuda.synchronize()
     st = ctx.get_stats()
     ctx.set_timing(False)
+    # one Laplace point per call (n_D = n_T): makes the integral re-computation per call visible
+    D1 = Dn[:w.nT].contiguous()
+    J1 = torch.empty_like(D1)
+    K1 = torch.empty_like(D1)
+    ctx.jk_build(D1, J1, K1)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    ctx.jk_build(D1, J1, K1)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    single_point = {"n_D": int(w.nT), "ms": e0.elapsed_time(e1), "builds_per_s": w.nT / (e0.elapsed_time(e1) * 1e-3)}
     Q = ctx.get_schwarz()
     ints = kept_integrals(Q, w.basis.l, w.schwarz_tau)
     digest_flops_alg = 20.0 * nD * ints                  # 2 J + 8 K FMAs per unique integral and density
@@ -290,7 +301,8 @@ def main():
                       "tau_schwarz": w.schwarz_tau, "shell_quartets_kept": nq_kept, "unique_integrals_kept": ints,
                       "l2": "inputs_larger_than_L2 (D, J, K are %.0f MB each)" % (8e-6 * nD * N * N),
                       "setup_outside_timed_region": "basis upload, shell pairs, Schwarz, work lists (geometry-frozen)",
-                      "laplace_grid": "library minimax" if wts is not None else "placeholder linspace (cost is value-independent)"},
+                      "laplace_grid": "library minimax" if wts is not None else "placeholder linspace (cost is value-independent)",
+                      "one_laplace_point_per_call": single_point},
            "clocks": clocks,
            "e2e": {"value": whole_job_builds_per_s(nD, world, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                    "ms_per_step": ms_e2e},
