@@ -142,7 +142,7 @@ class VRR:
         for e, ie in eidx.items():
             for f, jf in fidx.items():
                 v = self.node(e, f, 0)
-                self.lines.append("acc[%d] += %s;" % (ie * nf + jf, v))
+                self.lines.append("sink.template put<%d>(%s);" % (ie * nf + jf, v))
         return self.lines, len(eidx), nf
 
 
@@ -200,6 +200,7 @@ def main(out_dir):
             hdr.append("    " + ln)
         hdr.append("  }")
         hdr.append("};")
+    hdr.append("struct AccSink { double* __restrict__ acc; template<int I> LTJK_HD void put(const double v) { acc[I] += v; } };")
     hdr.append("template<int LA,int LB,int LC,int LD> struct Vrr;")
     stats = []
     for ib_, (la, lb) in enumerate(PAIR_CLASSES):
@@ -211,6 +212,20 @@ def main(out_dir):
             stats.append(((la, lb, lc, ld), g.n, ne * nf))
             hdr.append("template<> struct Vrr<%d,%d,%d,%d> {" % (la, lb, lc, ld))
             hdr.append("  static constexpr int NE = %d, NF = %d, NNODE = %d;" % (ne, nf, g.n))
+            # the targets are handed, in increasing index order, to a sink: `AccSink` adds them to a per-thread array
+            # (one thread per quartet), the cooperative kernels reduce them across the lanes of a half-warp instead
+            hdr.append("  template<class SINK> LTJK_HD static void run_t(const double* __restrict__ F, "
+                       "const double PAx, const double PAy, const double PAz, "
+                       "const double WPx, const double WPy, const double WPz, "
+                       "const double QCx, const double QCy, const double QCz, "
+                       "const double WQx, const double WQy, const double WQz, "
+                       "const double oo2p, const double oo2q, const double oo2pq, "
+                       "const double rp, const double rq, SINK& sink) {")
+            hdr.append("    (void)PAx;(void)PAy;(void)PAz;(void)WPx;(void)WPy;(void)WPz;(void)QCx;(void)QCy;(void)QCz;"
+                       "(void)WQx;(void)WQy;(void)WQz;(void)oo2p;(void)oo2q;(void)oo2pq;(void)rp;(void)rq;")
+            for ln in body:
+                hdr.append("    " + ln)
+            hdr.append("  }")
             hdr.append("  LTJK_HD static void run(const double* __restrict__ F, "
                        "const double PAx, const double PAy, const double PAz, "
                        "const double WPx, const double WPy, const double WPz, "
@@ -218,10 +233,8 @@ def main(out_dir):
                        "const double WQx, const double WQy, const double WQz, "
                        "const double oo2p, const double oo2q, const double oo2pq, "
                        "const double rp, const double rq, double* __restrict__ acc) {")
-            hdr.append("    (void)PAx;(void)PAy;(void)PAz;(void)WPx;(void)WPy;(void)WPz;(void)QCx;(void)QCy;(void)QCz;"
-                       "(void)WQx;(void)WQy;(void)WQz;(void)oo2p;(void)oo2q;(void)oo2pq;(void)rp;(void)rq;")
-            for ln in body:
-                hdr.append("    " + ln)
+            hdr.append("    AccSink s{acc};")
+            hdr.append("    run_t(F, PAx, PAy, PAz, WPx, WPy, WPz, QCx, QCy, QCz, WQx, WQy, WQz, oo2p, oo2q, oo2pq, rp, rq, s);")
             hdr.append("  }")
             hdr.append("};")
     hdr.append("} // namespace ltjk_gen")

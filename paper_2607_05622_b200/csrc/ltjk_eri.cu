@@ -139,6 +139,145 @@ __global__ void __launch_bounds__(64, 4) eri_panel_kernel(const EriArgs g)
                     P[a * sI + b * sJ + cc * sK + d] = scale * out[((a * NB + b) * NC + cc) * ND + d];
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// a6 + a7, cooperative variant for the classes whose contracted VRR targets do not fit a thread (NE*NF >= 256:
+// (dp|dp), (dd|pp), (dd|dp), (dd|dd)).  The one-thread-per-quartet kernel keeps those targets, the HRR scratch and
+// its spills in ~15-34 KB of local memory per thread and is bound by DRAM traffic (profiles/r1_eri_classes_ncu.txt).
+// Here a half-warp owns one contracted quartet: lane p evaluates primitive quartet p (Boys + VRR), the 16 partial
+// values of every target are summed by a reduce-scatter over the half-warp (15 shuffle-adds per 16 targets) into a
+// shared-memory [e0|f0] block, and both HRR stages run from shared memory with the columns / rows dealt to the lanes.
+template <int NTOT>
+struct CoopSink {
+    double buf[16];
+    double* __restrict__ accS;
+    unsigned hmask;
+    int l16;
+    bool first;
+    template <int I>
+    __device__ __forceinline__ void put(const double v)
+    {
+        buf[I & 15] = v;
+        if ((I & 15) == 15 || I == NTOT - 1) flush<(I >> 4), (I & 15) + 1>();
+    }
+    template <int G, int N>
+    __device__ __forceinline__ void flush()
+    {
+#pragma unroll
+        for (int i = N; i < 16; ++i) buf[i] = 0.0;
+        const bool b3 = l16 & 8, b2 = l16 & 4, b1 = l16 & 2, b0 = l16 & 1;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const double keep = b3 ? buf[i + 8] : buf[i], send = b3 ? buf[i] : buf[i + 8];
+            buf[i] = keep + __shfl_xor_sync(hmask, send, 8);
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const double keep = b2 ? buf[i + 4] : buf[i], send = b2 ? buf[i] : buf[i + 4];
+            buf[i] = keep + __shfl_xor_sync(hmask, send, 4);
+        }
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const double keep = b1 ? buf[i + 2] : buf[i], send = b1 ? buf[i] : buf[i + 2];
+            buf[i] = keep + __shfl_xor_sync(hmask, send, 2);
+        }
+        {
+            const double keep = b0 ? buf[1] : buf[0], send = b0 ? buf[0] : buf[1];
+            buf[0] = keep + __shfl_xor_sync(hmask, send, 1);
+        }
+        if (l16 < N) {                       // lane l16 now holds the contracted target G*16 + l16
+            if (first) accS[G * 16 + l16] = buf[0];
+            else accS[G * 16 + l16] += buf[0];
+        }
+    }
+};
+
+constexpr int kCoopThreads = 128;            // 8 half-warps = 8 quartets per CTA
+
+template <int LA, int LB, int LC, int LD>
+__global__ void __launch_bounds__(kCoopThreads, 1) eri_panel_coop_kernel(const EriArgs g)
+{
+    using V = ltjk_gen::Vrr<LA, LB, LC, LD>;
+    using HB = ltjk_gen::Hrr<LA, LB>;
+    using HK = ltjk_gen::Hrr<LC, LD>;
+    constexpr int L = LA + LB + LC + LD;
+    constexpr int NE = V::NE, NF = V::NF, NAB = HB::NAB, NCD = HK::NAB;
+    constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
+    constexpr int QS = NE * NF + NAB * NF;                  // doubles of shared memory per quartet
+    extern __shared__ __align__(16) double coop_sm[];
+    const int lane = threadIdx.x & 31, l16 = lane & 15, hw = threadIdx.x >> 4;
+    const unsigned hmask = (lane & 16) ? 0xffff0000u : 0x0000ffffu;
+    double* __restrict__ accS = coop_sm + hw * QS;
+    double* __restrict__ t1S = accS + NE * NF;
+
+    const SubChunk sc_ = g.subs[blockIdx.y];
+    const int ra = max(sc_.r0, g.ca), rb = min(sc_.r1, g.cb_);
+    const long long t = (long long)blockIdx.x * (kCoopThreads / 16) + hw;
+    const int r = ra + (int)(t / g.qn);
+    if (r >= rb) return;                                      // the whole half-warp leaves together
+    int q = (int)(t % g.qn);
+    const int sd = q % g.mL; q /= g.mL;
+    const int sc = q % g.mK; q /= g.mK;
+    const int sb = q % g.mJ;
+    const int sa = q / g.mJ;
+    const DevTables& T = g.t;
+    const int I = sc_.I, J = sc_.J, K = T.pair_I[r], Lb = T.pair_J[r];
+    if (sa >= T.blk_nsh[I] || sb >= T.blk_nsh[J] || sc >= T.blk_nsh[K] || sd >= T.blk_nsh[Lb]) return;
+    const int A = T.blk_sh0[I] + sa, B = T.blk_sh0[J] + sb, C = T.blk_sh0[K] + sc, D = T.blk_sh0[Lb] + sd;
+    const int nJ = T.blk_nao[J], nK = T.blk_nao[K], nL = T.blk_nao[Lb];
+    const long long base = sc_.base + (T.koff[r] - T.koff[sc_.r0]) * (long long)(T.blk_nao[I] * nJ);
+    double* __restrict__ P = g.panel + base + ((long long)(sa * NA) * nJ + sb * NB) * (nK * nL) + (sc * NC) * nL + sd * ND;
+    const int sI = nJ * nK * nL, sJ = nK * nL, sK = nL;
+
+    const double qq = T.schwarz[(size_t)A * T.nshell + B] * T.schwarz[(size_t)C * T.nshell + D];
+    if (qq < g.tau) {
+        for (int e = l16; e < NA * NB * NC * ND; e += 16) {
+            const int d = e % ND, cc = (e / ND) % NC, b = (e / (ND * NC)) % NB, a = e / (ND * NC * NB);
+            P[a * sI + b * sJ + cc * sK + d] = 0.0;
+        }
+        return;
+    }
+    double scale = 1.0;
+    if (I == J) scale *= 0.5;
+    if (K == Lb) scale *= 0.5;
+    if (r == sc_.rIJ) scale *= 0.5;
+
+    const double* __restrict__ bra = T.pair_rec + ((size_t)A * T.nshell + B) * T.rec_stride;
+    const double* __restrict__ ket = T.pair_rec + ((size_t)C * T.nshell + D) * T.rec_stride;
+    const int nb = (int)bra[3], nk = (int)ket[3], nprimq = nb * nk;
+    for (int p0 = 0; p0 < nprimq; p0 += 16) {
+        const int p = p0 + l16;
+        const bool active = p < nprimq;
+        const double* bp = bra + kPairHeader + (active ? p / nk : 0) * kPrimStride;
+        const double* kp = ket + kPairHeader + (active ? p % nk : 0) * kPrimStride;
+        const double pp = bp[0], qv = kp[0];
+        const double pq = pp + qv, ipq = 1.0 / pq;
+        double pref = bp[7] * kp[7] * 34.986836655249725693 /* 2 pi^{5/2} */ / (pp * qv * sqrt(pq));
+        if (!active || fabs(pref) < kPrimCut) pref = 0.0;     // the VRR is linear in F: zero F = zero contribution
+        const double PQx = bp[1] - kp[1], PQy = bp[2] - kp[2], PQz = bp[3] - kp[3];
+        const double rho = pp * qv * ipq;
+        double F[L + 1];
+        boys_scaled<L>(rho * (PQx * PQx + PQy * PQy + PQz * PQz), pref, T.boys, F);
+        const double wp = -qv * ipq, wq = pp * ipq;
+        CoopSink<NE * NF> sink;
+        sink.accS = accS; sink.hmask = hmask; sink.l16 = l16; sink.first = (p0 == 0);
+        V::run_t(F, bp[4], bp[5], bp[6], wp * PQx, wp * PQy, wp * PQz, kp[4], kp[5], kp[6], wq * PQx, wq * PQy, wq * PQz,
+                 0.5 / pp, 0.5 / qv, 0.5 * ipq, qv * ipq /* rho/p */, pp * ipq /* rho/q */, sink);
+        __syncwarp(hmask);
+    }
+    // HRR on the bra for every ket component (columns dealt to the lanes), then on the ket for every (a,b) row
+    for (int jf = l16; jf < NF; jf += 16) HB::run(accS + jf, NF, t1S + jf, NF, bra[0], bra[1], bra[2]);
+    __syncwarp(hmask);
+    for (int iab = l16; iab < NAB; iab += 16) {
+        double o[NCD];
+        HK::run(t1S + iab * NF, 1, o, 1, ket[0], ket[1], ket[2]);
+        double* __restrict__ Pab = P + (iab / NB) * sI + (iab % NB) * sJ;
+#pragma unroll
+        for (int cc = 0; cc < NC; ++cc)
+#pragma unroll
+            for (int d = 0; d < ND; ++d) Pab[cc * sK + d] = scale * o[cc * ND + d];
+    }
+}
+
 static const int kClsLa[6] = {0, 1, 1, 2, 2, 2}, kClsLb[6] = {0, 0, 1, 0, 1, 2};
 
 template <int CB, int CK>
@@ -146,6 +285,23 @@ static int launch_cls(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
 {
     constexpr int la[6] = {0, 1, 1, 2, 2, 2}, lb[6] = {0, 0, 1, 0, 1, 2};
     if constexpr (CK <= CB) {
+        using V = ltjk_gen::Vrr<la[CB], lb[CB], la[CK], lb[CK]>;
+        if constexpr (lb[CB] > 0 && lb[CK] > 0 && V::NE * V::NF >= 256) {
+            constexpr int QS = V::NE * V::NF + ltjk_gen::Hrr<la[CB], lb[CB]>::NAB * V::NF;
+            constexpr int smem = (kCoopThreads / 16) * QS * (int)sizeof(double);
+            static bool attr = false;
+            if (!attr) {
+                LTJK_CUDA(c, cudaFuncSetAttribute(eri_panel_coop_kernel<la[CB], lb[CB], la[CK], lb[CK]>,
+                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+                attr = true;
+            }
+            const long long nq = (long long)maxkets * g.qn;
+            const int per = kCoopThreads / 16;
+            eri_panel_coop_kernel<la[CB], lb[CB], la[CK], lb[CK]>
+                <<<dim3((unsigned)((nq + per - 1) / per), nsub), kCoopThreads, smem, c->eri_stream>>>(g);
+            LTJK_CUDA(c, cudaGetLastError());
+            return LTJK_OK;
+        }
         const long long nthr = (long long)maxkets * g.qn;
         const int bs = 64;
         static bool carve = false;      // no shared memory used: give the whole unified cache to L1 (local-memory spills)
