@@ -140,8 +140,8 @@ __global__ void __launch_bounds__(64, 4) eri_panel_kernel(const EriArgs g)
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// a6 + a7, cooperative variant for the classes whose contracted VRR targets do not fit a thread (NE*NF >= 256:
-// (dp|dp), (dd|pp), (dd|dp), (dd|dd)).  The one-thread-per-quartet kernel keeps those targets, the HRR scratch and
+// a6 + a7, cooperative variant for the classes whose contracted VRR targets do not fit a thread (l_b, l_d > 0 and
+// NE*NF >= 128: (dp|pp), (dp|dp), (dd|pp), (dd|dp), (dd|dd)).  The one-thread-per-quartet kernel keeps those targets, the HRR scratch and
 // its spills in ~15-34 KB of local memory per thread and is bound by DRAM traffic (profiles/r1_eri_classes_ncu.txt).
 // Here a half-warp owns one contracted quartet: lane p evaluates primitive quartet p (Boys + VRR), the 16 partial
 // values of every target are summed by a reduce-scatter over the half-warp (15 shuffle-adds per 16 targets) into a
@@ -286,7 +286,9 @@ static int launch_cls(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
     constexpr int la[6] = {0, 1, 1, 2, 2, 2}, lb[6] = {0, 0, 1, 0, 1, 2};
     if constexpr (CK <= CB) {
         using V = ltjk_gen::Vrr<la[CB], lb[CB], la[CK], lb[CK]>;
-        if constexpr (lb[CB] > 0 && lb[CK] > 0 && V::NE * V::NF >= 256) {
+        // measured on B200: worth it from 128 targets up ((pp|pp) with 81 is faster one thread per quartet, and so
+        // are the l_d = 0 classes)
+        if constexpr (lb[CB] > 0 && lb[CK] > 0 && V::NE * V::NF >= 128) {
             constexpr int QS = V::NE * V::NF + ltjk_gen::Hrr<la[CB], lb[CB]>::NAB * V::NF;
             constexpr int smem = (kCoopThreads / 16) * QS * (int)sizeof(double);
             static bool attr = false;
