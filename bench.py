@@ -170,6 +170,9 @@ def main():
 
     import torch
     import torch.distributed as dist
+    from paper_2607_05622_b200 import build as _build
+    if rank == 0 and not _build.LIB.exists():
+        _build.build()          # in-tree build of libltjk.so (the driver normally did this through build())
     from paper_2607_05622_b200 import ltjk
     from paper_2607_05622_b200.inputs import make_workload
 

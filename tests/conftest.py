@@ -33,3 +33,11 @@ def spd_basis():
     xyz = np.array([[0.0, 0.1, -0.2], [1.9, 0.3, 0.4], [-0.7, 2.1, 1.0]])
     sh = [(0, [0.9, 0.3], [0.6, 0.4]), (1, [0.7, 0.25], [0.6, 0.4]), (2, [0.8, 0.35], [0.6, 0.4])]
     return custom_basis(xyz, [sh, sh, sh])
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _built_library():
+    """The CUDA library is built in-tree (incremental, a no-op when up to date); tests never run against a stale or
+    missing libltjk.so.  nvcc cross-compiles without a GPU, so this also holds for the CPU tier."""
+    from paper_2607_05622_b200 import build
+    build.build()
