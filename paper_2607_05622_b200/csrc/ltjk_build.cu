@@ -132,7 +132,7 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     }
     maxpanel *= maxpanel;
 
-    // ---- panel staging ring: L2-sized by default, never below one panel
+    // ---- panel staging ring (two halves), never below one panel per half
     size_t freeb = 0, totb = 0;
     LTJK_CUDA(c, cudaMemGetInfo(&freeb, &totb));
     // Default 8 GiB (two 4 GiB halves), at most a quarter of the free memory: measured on B200, launches that fill

@@ -12,7 +12,7 @@
 //     view 4  KIL: rows (i,l) cols (j,k)  B = D[(j,k)] -> K[(i,l)] ; partner B = D[(k,j)] -> K[(l,i)]
 //     view 5  KJL: rows (j,l) cols (i,k)  B = D[(i,k)] -> K[(j,l)] ; partner B = D[(k,i)] -> K[(l,j)]
 // (the 2 J and 8 K images of a canonical quartet; for D != D^T all eight K images are distinct).
-// One CTA owns a 64-row tile of one output block for all (<= 192) densities, keeps it in registers over a RUN of
+// One CTA owns a 128-row tile of one output block for all (<= 192) densities, keeps it in registers over a RUN of
 // panels sharing that output block, and flushes once with coalesced fp64 reductions.
 #include "ltjk_internal.h"
 #include <cstdio>

@@ -1,10 +1,10 @@
 // ltjk_eri.cu -- steps a2 (shell-pair records, Schwarz bounds), a6+a7 (Boys + OS/HGP shell quartets) as kernels.
 //
-// Integral panels.  A canonical block quartet (IJ|KL) (blocks = l-homogeneous groups of ~16 AOs, see
+// Integral panels.  A canonical block quartet (IJ|KL) (blocks = l-homogeneous groups of 16-24 AOs, see
 // ltjk_internal.h) owns a dense panel  P[i][j][k][l] = s * (ij|kl),  i in I, j in J, k in K, l in L,
 // s = 1/2 per coincidence I==J, K==L, (IJ)==(KL)  (the "canonical-fold multiplicity" of PAPER.md:L320-322 Eq. 25,
-// DESIGN.md reading A4, applied at block level).  Panels live in an L2-sized staging ring, are written here by one
-// thread per contracted shell quartet (the paper's mapping) and are consumed by the
+// DESIGN.md reading A4, applied at block level).  Panels live in a two-half staging ring, are written here by one
+// thread per contracted shell quartet (the paper's mapping; a half-warp for the heaviest classes) and consumed by the
 // digestion kernels (ltjk_digest.cu) before the ring is reused: integrals never form a stored N^4 object.
 // Shell quartets with Q_AB Q_CD < tau (reading A9) are written as zeros.
 #include "ltjk_internal.h"

@@ -11,7 +11,7 @@ namespace ltjk {
 constexpr int kDigestRows = 128;   // output rows per digestion CTA (ltjk_digest.cu) = row-tile height of the work items
 
 // ---- geometry-frozen device tables (built by ltjk_build_shell_pairs, reused by every jk_build) ----------------
-// Shells are re-ordered internally by angular momentum and cut into l-homogeneous BLOCKS of ~16 AOs; block
+// Shells are re-ordered internally by angular momentum and cut into l-homogeneous BLOCKS of 16-24 AOs; block
 // pairs (I>=J) are ranked class-major ((ss),(ps),(pp),(ds),(dp),(dd)), so that every canonical block quartet
 // (IJ|KL), rank(IJ) >= rank(KL), has bra class >= ket class and every panel is class-homogeneous.
 struct DevTables {
@@ -105,7 +105,7 @@ struct ltjk_ctx {
     unsigned char* d_chunkmask = nullptr; // one byte per (item, chunk): bit w = sub-tile of consumer warp w not entirely screened
     long long n_maskbits = 0;
     long long n_items = 0;
-    double* d_panel = nullptr;            // integral panel staging ring (L2-sized)
+    double* d_panel = nullptr;            // integral panel staging ring (two halves)
     long long panel_cap = 0;              // doubles (both halves)
     long long panel_half = 0;             // doubles per half: chunk c lives in half c&1 (ERI of c+1 overlaps digest of c)
     cudaStream_t eri_stream = nullptr;    // stream of the ERI kernels (== stream when timing serialises the phases)
