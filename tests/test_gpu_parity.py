@@ -332,3 +332,18 @@ def test_laplace_cascade_closure(torch_cuda, small):
     ctx.laplace_fock(J[:4].contiguous(), K[:4].contiguous(), dev(w.C_occ), Fo)
     torch.cuda.synchronize()
     assert relerr(Fo.cpu().numpy(), Fr[:, :w.nocc, :w.nocc]) < 1e-12
+
+
+def test_three_and_four_primitive_contractions(torch_cuda):
+    """Contraction depths other than the benchmark's 2: 3- and 4-primitive shells give 81 / 144 / 256 primitive
+    quartets per contracted quartet, i.e. several 16-lane passes of the cooperative ERI kernel and long primitive
+    loops in the per-thread kernels."""
+    xyz = np.array([[0.0, 0.1, -0.2], [1.7, -0.4, 0.5], [-0.9, 1.8, 0.7]])
+    sh3 = [(0, [2.1, 0.7, 0.25], [0.3, 0.5, 0.3]), (1, [1.5, 0.5, 0.2], [0.25, 0.5, 0.35]), (2, [1.1, 0.45, 0.2], [0.3, 0.4, 0.4])]
+    sh4 = [(1, [2.5, 0.9, 0.35, 0.15], [0.2, 0.3, 0.3, 0.2]), (2, [1.4, 0.6, 0.3, 0.15], [0.2, 0.3, 0.3, 0.2])]
+    b = custom_basis(xyz, [sh3, sh4, sh3])
+    D = random_densities(b.nao, 3, seed=41)
+    ctx = make_ctx(b, tau=0.0)
+    J, K = gpu_jk(torch_cuda, ctx, D)
+    Jr, Kr = O.jk_definition(O.eri_tensor(b), D)
+    assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
