@@ -102,27 +102,38 @@ def oracle_sample(w, D, target_s=15.0):
             s += nf[p] * float(nf[:p + 1][keep].sum())
         return s
 
-    # start in the middle of the pair list (typical cost), take pairs until the estimated time is reached
+    # Bra shell pairs from the middle of the pair list (typical cost).  Every oracle call has a fixed cost (density-
+    # fastest copies of D, per-thread J/K buffers and their reduction) that a whole sweep pays once, so the sweep time is
+    # extrapolated from a linear fit t = t0 + rate * integrals over calls of growing size, not from a plain ratio.
     p0 = npair // 2
     n = 1
-    t_used, ints_done = 0.0, 0.0
+    t_used = 0.0
+    pts = []
     while True:
         p1 = min(p0 + n, npair)
         t = time.perf_counter()
         O.jk_folded(b, D, w.schwarz_tau, pair_range=(p0, p1), Q=Q)
         dt = time.perf_counter() - t
         t_used += dt
-        ints_done += ints_of(p0, p1)
+        pts.append((ints_of(p0, p1), dt))
         if t_used >= target_s or p1 >= npair:
             break
-        rate = dt / max(n, 1)
         p0 = p1
-        n = int(max(1, min((target_s - t_used) / max(rate, 1e-6), 4 * n)))
-    sweep_s = t_used * total_ints / max(ints_done, 1.0)
+        n = int(max(2, min(4 * n, 64 * n if dt < 0.05 * target_s else 4 * n)))
+    x = np.array([q[0] for q in pts])
+    y = np.array([q[1] for q in pts])
+    if len(pts) >= 2 and x.max() > x.min():
+        rate, t0 = np.polyfit(x, y, 1)
+        if rate <= 0:
+            rate, t0 = y[-1] / x[-1], 0.0
+        t0 = max(t0, 0.0)
+    else:
+        rate, t0 = y[-1] / max(x[-1], 1.0), 0.0
+    sweep_s = t0 + rate * total_ints
     return {"value": D.shape[0] / sweep_s, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle",
-            "sample": "oracle O6 (folded MD loop, all %d densities) on a run of bra shell pairs holding %.3g of the %.3g "
-                      "kept unique integrals, %.1f s of CPU time, scaled to the whole sweep" %
-                      (D.shape[0], ints_done, total_ints, t_used)}
+            "sample": "oracle O6 (folded MD loop, all %d densities) on %d runs of bra shell pairs holding %.3g of the %.3g "
+                      "kept unique integrals, %.1f s of CPU time; sweep time from the linear fit t = %.2f s + %.3g s/integral" %
+                      (D.shape[0], len(pts), float(x.sum()), total_ints, t_used, t0, rate)}
 
 
 def run_reference(args, rank, world):
