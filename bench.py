@@ -102,38 +102,34 @@ def oracle_sample(w, D, target_s=15.0):
             s += nf[p] * float(nf[:p + 1][keep].sum())
         return s
 
-    # Bra shell pairs from the middle of the pair list (typical cost).  Every oracle call has a fixed cost (density-
-    # fastest copies of D, per-thread J/K buffers and their reduction) that a whole sweep pays once, so the sweep time is
-    # extrapolated from a linear fit t = t0 + rate * integrals over calls of growing size, not from a plain ratio.
-    p0 = npair // 2
-    n = 1
-    t_used = 0.0
-    pts = []
-    while True:
-        p1 = min(p0 + n, npair)
+    # Every oracle call has a fixed cost (density-fastest copies of D, per-thread J/K buffers and their reduction) that a
+    # whole sweep pays once: it is measured by a call with an empty pair range; the per-integral rate comes from one
+    # call over a run of bra shell pairs from the middle of the pair list (typical cost), sized by a short calibration
+    # call to use the rest of the time budget.  sweep time = fixed + rate * (kept unique integrals).
+    def call(pa, pb):
         t = time.perf_counter()
-        O.jk_folded(b, D, w.schwarz_tau, pair_range=(p0, p1), Q=Q)
-        dt = time.perf_counter() - t
-        t_used += dt
-        pts.append((ints_of(p0, p1), dt))
-        if t_used >= target_s or p1 >= npair:
-            break
-        p0 = p1
-        n = int(max(2, min(4 * n, 64 * n if dt < 0.05 * target_s else 4 * n)))
-    x = np.array([q[0] for q in pts])
-    y = np.array([q[1] for q in pts])
-    if len(pts) >= 2 and x.max() > x.min():
-        rate, t0 = np.polyfit(x, y, 1)
-        if rate <= 0:
-            rate, t0 = y[-1] / x[-1], 0.0
-        t0 = max(t0, 0.0)
-    else:
-        rate, t0 = y[-1] / max(x[-1], 1.0), 0.0
-    sweep_s = t0 + rate * total_ints
+        O.jk_folded(b, D, w.schwarz_tau, pair_range=(pa, pb), Q=Q)
+        return time.perf_counter() - t
+
+    t_fixed = call(0, 0)
+    p0 = npair // 2
+    t_cal = call(p0, min(p0 + 4, npair))
+    i_cal = ints_of(p0, min(p0 + 4, npair))
+    rate_cal = max(t_cal - t_fixed, 1e-3) / max(i_cal, 1.0)
+    budget = max(target_s - t_fixed - t_cal - t_fixed, 2.0)          # the big call pays the fixed cost again
+    n = 4
+    while p0 + 4 + n < npair and ints_of(p0 + 4, p0 + 4 + n) * rate_cal < budget and n < 65536:
+        n *= 2
+    pa, pb = p0 + 4, min(p0 + 4 + n, npair)
+    t_big = call(pa, pb)
+    i_big = ints_of(pa, pb)
+    rate = max(t_big - t_fixed, 1e-6) / max(i_big, 1.0)
+    t_used = t_fixed + t_cal + t_big
+    sweep_s = t_fixed + rate * total_ints
     return {"value": D.shape[0] / sweep_s, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle",
-            "sample": "oracle O6 (folded MD loop, all %d densities) on %d runs of bra shell pairs holding %.3g of the %.3g "
-                      "kept unique integrals, %.1f s of CPU time; sweep time from the linear fit t = %.2f s + %.3g s/integral" %
-                      (D.shape[0], len(pts), float(x.sum()), total_ints, t_used, t0, rate)}
+            "sample": "oracle O6 (folded MD loop, all %d densities): %.1f s of CPU time; fixed cost per call %.2f s (empty "
+                      "pair range), then %.3g of the %.3g kept unique integrals in %.2f s -> %.3g s per integral; sweep = "
+                      "fixed + rate x all integrals" % (D.shape[0], t_used, t_fixed, i_big, total_ints, t_big, rate)}
 
 
 def run_reference(args, rank, world):
