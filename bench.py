@@ -251,7 +251,10 @@ def main():
     t0 = time.perf_counter()
     e0.record(stream)
     for _ in range(n_e2e):
+        tc = time.perf_counter()
         ctx.sweep_host(hCo, hCv, heo, hev, hT, tau, hJ, hK)
+        if rank == 0:
+            print("e2e sweep_host call: %.1f ms" % ((time.perf_counter() - tc) * 1e3), file=sys.stderr)
     e1.record(stream)
     barrier()
     ms_e2e = e0.elapsed_time(e1) / n_e2e
