@@ -3,8 +3,8 @@
 //   1/x ~ sum_a w_a exp(-x tau_a),  minimise  max_{x in [xmin,xmax]} |1/x - sum_a w_a exp(-x tau_a)|.
 //
 // Host code, quadruple precision (__float128): the problem is solved on [1,R], R = xmax/xmin, and scaled
-// (tau = tau^/xmin, w = w^/xmin).  Method (this library's own; the CPU oracle uses a different start and
-// 120-digit arithmetic, reading A8):
+// (tau = tau^/xmin, w = w^/xmin).  Method (this library's own code; the CPU oracle is an independent Python/mpmath
+// implementation in 80-digit arithmetic, reading A8):
 //   1. start on a wide interval [1,R0]: Levenberg-Marquardt least squares in (log tau, log w) on a logarithmic
 //      grid, from the trapezoid rule for 1/x = int exp(-x e^s) e^s ds; accepted only if its error curve has
 //      2k+1 alternating extrema (else another R0 is tried);
@@ -17,8 +17,6 @@
 #include <algorithm>
 #include <cmath>
 #include <vector>
-#include <cstdio>
-#include <cstdlib>
 
 namespace {
 
@@ -241,19 +239,15 @@ bool minimax(int k, real R, Grid& g, real& delta)
         Grid s;
         ls_start(k, R0, s);
         vec xs = find_extrema(s, R0, 3000);
-        const bool dbg = getenv("LTJK_LAPLACE_DEBUG") != nullptr;
-        if (dbg) fprintf(stderr, "laplace k=%d c=%.1f R0=%.4g extrema=%d (need %d)\n", k, c, (double)R0, (int)xs.size(), 2 * k + 1);
         if ((int)xs.size() != 2 * k + 1 || !alternates(s, xs)) continue;
         real Rc = R0;
         bool ok = remez(k, Rc, s, xs, delta);
-        if (dbg) fprintf(stderr, "  remez at R0: ok=%d delta=%.4e\n", (int)ok, (double)delta);
         while (ok && Rc > R) {
             real Rn = Rc / 1.2Q;
             if (Rn < R) Rn = R;
             for (auto& x : xs) x = qexp(qlog(x) * qlog(Rn) / qlog(Rc));
             Rc = Rn;
             ok = remez(k, Rc, s, xs, delta);
-            if (dbg) fprintf(stderr, "  remez at R=%.5g: ok=%d delta=%.4e\n", (double)Rc, (int)ok, (double)delta);
         }
         if (ok) { g = s; return true; }
     }
