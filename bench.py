@@ -315,7 +315,9 @@ def main():
                       "l2": "inputs_larger_than_L2 (D, J, K are %.0f MB each)" % (8e-6 * nD * N * N),
                       "setup_outside_timed_region": "basis upload, shell pairs, Schwarz, work lists (geometry-frozen)",
                       "laplace_grid": "library minimax" if wts is not None else "placeholder linspace (cost is value-independent)",
-                      "one_laplace_point_per_call": single_point},
+                      "one_laplace_point_per_call": single_point,
+                      "gpu": torch.cuda.get_device_name(local), "hbm_copy_gbs_measured": ctx.bench_copy_peak(),
+                      "dfma_peak_tflops_measured": peak_tf},
            "clocks": clocks,
            "e2e": {"value": whole_job_builds_per_s(nD, world, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                    "ms_per_step": ms_e2e},

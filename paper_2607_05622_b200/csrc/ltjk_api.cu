@@ -219,6 +219,13 @@ int ltjk_create(ltjk_ctx** out, int device, void* cuda_stream)
     if (!c) return LTJK_ENOMEM;
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
+    {   // keep the stream-ordered allocations (transform scratch, host-entry staging) cached between calls
+        cudaMemPool_t pool = nullptr;
+        if (cudaDeviceGetDefaultMemPool(&pool, device) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+    }
     if (cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return LTJK_ECUDA; }
     c->eri_stream = c->own_stream;
     for (int i = 0; i < 2; ++i) {
