@@ -247,6 +247,75 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
 
     // ===================== consumer warpgroups =====================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
+    if constexpr (TN <= 5) {
+    // thread tile 8 rows x 2 TN columns: the two half-warps of warp w own rows 16w..16w+7 and 16w+8..16w+15, lane l16
+    // owns the column pairs (2 l16, 2 l16 + 1) + 32 t.  Per k: 4 LDS.128 for A (two addresses per warp) and TN LDS.128
+    // for B, against 8 + TN LDS.64 with a 16 x TN tile (measured +4 % on the isolated loop)
+    const int wrow = w * kTM;
+    const int trow = wrow + (lane >> 4) * 8;
+    const int l16 = lane & 15;
+    for (int vi = blockIdx.x; vi < nvirt; vi += gridDim.x) {
+        const ItemCtx c = load_item(g, vi, ncolblk, 32 * TN);
+        const DigestItem& it = c.it;
+        const int view = it.view;
+        const int total_chunks = it.nnz;
+        const bool warp_active = it.rowtile * kMT + wrow < c.nrows;   // ragged last tile: idle warps skip the DFMAs
+        double acc[8][2 * TN];
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+#pragma unroll
+            for (int t = 0; t < 2 * TN; ++t) acc[r][t] = 0.0;
+
+        for (int q = 0; q < total_chunks; ++q, ++gch) {
+            const int st = gch % kStages;
+            mbar_wait(&S.full[st], (unsigned)((gch / kStages) & 1));
+            if (warp_active && ((S.cmask[st] >> w) & 1u)) {
+#pragma unroll
+                for (int k = 0; k < kKC; ++k) {
+                    const double2* ap = reinterpret_cast<const double2*>(&S.A[st][k][trow]);
+                    double a[8];
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) { const double2 v = ap[r]; a[2 * r] = v.x; a[2 * r + 1] = v.y; }
+                    double b[2 * TN];
+#pragma unroll
+                    for (int t = 0; t < TN; ++t) {
+                        const double2 v = *reinterpret_cast<const double2*>(&S.B[st][k][2 * l16 + 32 * t]);
+                        b[2 * t] = v.x; b[2 * t + 1] = v.y;
+                    }
+#pragma unroll
+                    for (int r = 0; r < 8; ++r)
+#pragma unroll
+                        for (int t = 0; t < 2 * TN; ++t) acc[r][t] = fma(a[r], b[t], acc[r][t]);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&S.empty[st]);
+        }
+
+        // flush: coalesced fp64 reductions into the density-fastest accumulators
+        if (warp_active) {
+            const double mult = (double)it.mult;
+            const bool partner = it.partner != 0;
+            double* __restrict__ Out = (view <= 1) ? g.Jt : g.Kt;
+            const int aoR1 = T.blk_ao0[c.R1], aoR2 = T.blk_ao0[c.R2];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                const int m = it.rowtile * kMT + trow + r;
+                if (m < c.nrows) {
+                    const int r1 = m / c.nR2, r2 = m % c.nR2;
+                    const size_t row = partner ? (size_t)(aoR2 + r2) * N + aoR1 + r1 : (size_t)(aoR1 + r1) * N + aoR2 + r2;
+                    double* o = Out + row * nDp + c.n0 + 2 * l16;
+#pragma unroll
+                    for (int t = 0; t < TN; ++t) {
+                        atomicAdd(o + 32 * t, mult * acc[r][2 * t]);
+                        atomicAdd(o + 32 * t + 1, mult * acc[r][2 * t + 1]);
+                    }
+                }
+            }
+        }
+    }
+    } else {
+        // TN = 6 (192 densities per column block): the 16 x TN tile measured faster there
     const int trow = w * kTM;
     for (int vi = blockIdx.x; vi < nvirt; vi += gridDim.x) {
         const ItemCtx c = load_item(g, vi, ncolblk, 32 * TN);
@@ -301,6 +370,7 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
                 }
             }
         }
+    }
     }
 }
 
