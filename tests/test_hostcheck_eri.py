@@ -1,5 +1,5 @@
 """Host logic tier: the generated Obara-Saika/HGP recurrences and the table-driven Boys evaluator of the CUDA path,
-compiled for the host by a TEST-ONLY shim (csrc/host_check.cpp), against the CPU oracle (McMurchie-Davidson).
+compiled for the host by a TEST-ONLY shim (tests/host_check.cpp, built into a temporary directory), against the CPU oracle (McMurchie-Davidson).
 Two different textbook recurrences agreeing to round-off is the main evidence that the integrals are right
 (SURVEY.md 8(c) P-E); the same comparison runs on the GPU in test_gpu_parity.py."""
 import ctypes
@@ -18,12 +18,12 @@ _dp = ctypes.POINTER(ctypes.c_double)
 
 
 @pytest.fixture(scope="module")
-def hc():
-    subprocess.check_call(["python", str(CSRC / "gen_eri.py"), str(CSRC / "gen")])
-    so = CSRC / "libltjk_hostcheck.so"
-    srcs = [CSRC / "host_check.cpp", CSRC / "eri_core.h", CSRC / "boys_table.h", CSRC / "gen" / "eri_gen.h"]
-    if not so.exists() or so.stat().st_mtime < max(s.stat().st_mtime for s in srcs):
-        subprocess.check_call(["g++", "-O1", "-std=c++17", "-shared", "-fPIC", "-o", str(so), str(CSRC / "host_check.cpp")])
+def hc(tmp_path_factory):
+    from paper_2607_05622_b200 import build
+    build.build()                                   # generates csrc/gen/eri_gen.h when missing or stale
+    so = tmp_path_factory.mktemp("hostcheck") / "libltjk_hostcheck.so"
+    subprocess.check_call(["g++", "-O1", "-std=c++17", "-shared", "-fPIC", "-I", str(CSRC), "-o", str(so),
+                           str(Path(__file__).resolve().parent / "host_check.cpp")])
     return ctypes.CDLL(str(so))
 
 
