@@ -25,8 +25,11 @@ import numpy as np
 ROOT = Path(__file__).resolve().parent
 sys.path.insert(0, str(ROOT))
 
-METRIC = "non-symmetric J/K builds/s (fp64) at 439 AO"
 UNIT = "builds/s"
+
+
+def metric_name(w):
+    return "non-symmetric J/K builds/s (fp64) at %d AO" % w.nao
 
 
 def kept_integrals(Q, l, tau):
@@ -81,82 +84,201 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
-def oracle_sample(w, D, target_s=15.0):
-    """Time the oracle (as it stands) on a bounded sample of the workload: a prefix of bra shell pairs of the folded
-    loop O6 with all nD densities, grown until ~target_s of CPU work; scaled by the kept-quartet share."""
+def pair_integrals(Q, l, tau):
+    """Per bra shell pair p (canonical order A(A+1)/2+B of the folded loop O6): number of kept unique integrals of its
+    quartets (p | q <= p).  Pure counting from the Schwarz bounds; used to scale oracle samples."""
+    nc = np.array([1, 3, 6])[np.asarray(l)]
+    ns = len(l)
+    iu = np.tril_indices(ns)
+    qv = Q[iu]
+    nf = (nc[iu[0]] * nc[iu[1]]).astype(np.float64)
+    out = np.zeros(len(qv))
+    step = 2048
+    for p0 in range(0, len(qv), step):
+        p1 = min(p0 + step, len(qv))
+        keep = (qv[None, :p1] * qv[p0:p1, None] >= tau) & (np.arange(p1)[None, :] <= np.arange(p0, p1)[:, None])
+        out[p0:p1] = nf[p0:p1] * (keep * nf[None, :p1]).sum(1)
+    return out
+
+
+def oracle_sample(w, D, target_s=15.0, nstrata=4):
+    """Time the oracle (as it stands) on a bounded, STRATIFIED sample of the workload: the bra shell-pair list of the
+    folded loop O6 is cut into `nstrata` strata of equal kept-integral share; a run of pairs from the middle of each
+    stratum is timed with all nD densities.  Whole-sweep time = fixed per-call cost + sum_s rate_s x integrals_s: an
+    EXTRAPOLATION (kind says so); the spread of the per-stratum rates is reported."""
     from oracle import oracle as O
     b = w.basis
     Q = O.schwarz(b)
     npair = b.nshell * (b.nshell + 1) // 2
-    nc = np.array([1, 3, 6])[b.l]
-    total_ints = kept_integrals(Q, b.l, w.schwarz_tau)
-    # integrals of bra pairs [p0,p1): bra pair p against kets q<=p
-    iu = np.tril_indices(b.nshell)
-    qv = Q[iu]
-    nf = (nc[iu[0]] * nc[iu[1]]).astype(np.float64)
+    pints = pair_integrals(Q, b.l, w.schwarz_tau)
+    cum = np.concatenate([[0.0], np.cumsum(pints)])
+    total_ints = float(cum[-1])
 
-    def ints_of(p0, p1):
-        s = 0.0
-        for p in range(p0, p1):
-            keep = qv[:p + 1] * qv[p] >= w.schwarz_tau
-            s += nf[p] * float(nf[:p + 1][keep].sum())
-        return s
-
-    # Every oracle call has a fixed cost (density-fastest copies of D, per-thread J/K buffers and their reduction) that a
-    # whole sweep pays once: it is measured by a call with an empty pair range; the per-integral rate comes from one
-    # call over a run of bra shell pairs from the middle of the pair list (typical cost), sized by a short calibration
-    # call to use the rest of the time budget.  sweep time = fixed + rate * (kept unique integrals).
     def call(pa, pb):
         t = time.perf_counter()
         O.jk_folded(b, D, w.schwarz_tau, pair_range=(pa, pb), Q=Q)
         return time.perf_counter() - t
 
-    t_fixed = call(0, 0)
-    p0 = npair // 2
-    t_cal = call(p0, min(p0 + 4, npair))
-    i_cal = ints_of(p0, min(p0 + 4, npair))
-    rate_cal = max(t_cal - t_fixed, 1e-3) / max(i_cal, 1.0)
-    budget = max(target_s - t_fixed - t_cal - t_fixed, 2.0)          # the big call pays the fixed cost again
-    n = 4
-    while p0 + 4 + n < npair and ints_of(p0 + 4, p0 + 4 + n) * rate_cal < budget and n < 65536:
-        n *= 2
-    pa, pb = p0 + 4, min(p0 + 4 + n, npair)
-    t_big = call(pa, pb)
-    i_big = ints_of(pa, pb)
-    rate = max(t_big - t_fixed, 1e-6) / max(i_big, 1.0)
-    t_used = t_fixed + t_cal + t_big
-    sweep_s = t_fixed + rate * total_ints
-    return {"value": D.shape[0] / sweep_s, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle",
-            "sample": "oracle O6 (folded MD loop, all %d densities): %.1f s of CPU time; fixed cost per call %.2f s (empty "
-                      "pair range), then %.3g of the %.3g kept unique integrals in %.2f s -> %.3g s per integral; sweep = "
-                      "fixed + rate x all integrals" % (D.shape[0], t_used, t_fixed, i_big, total_ints, t_big, rate)}
+    t_fixed = call(0, 0)                   # density-fastest copies of D, per-thread J/K buffers and their reduction
+    bounds = [int(np.searchsorted(cum, total_ints * k / nstrata)) for k in range(nstrata + 1)]
+    bounds[0], bounds[-1] = 0, npair
+    mids = [int(np.searchsorted(cum, total_ints * (k + 0.5) / nstrata)) for k in range(nstrata)]
+    # calibration: a short run in the first stratum sizes the samples to the time budget
+    pa = min(mids[0], npair - 1)
+    t_cal = call(pa, min(pa + 2, npair))
+    rate_cal = max(t_cal - t_fixed, 1e-3) / max(cum[min(pa + 2, npair)] - cum[pa], 1.0)
+    per = max((target_s - 2 * t_fixed - t_cal) / nstrata - t_fixed, 0.5)
+    rates, used, sampled = [], t_fixed + t_cal, 0.0
+    for k in range(nstrata):
+        pa = min(mids[k], npair - 1)
+        pb = int(np.searchsorted(cum, cum[pa] + per / rate_cal))
+        pb = max(pa + 1, min(pb, bounds[k + 1], npair))
+        t = call(pa, pb)
+        ints = max(cum[pb] - cum[pa], 1.0)
+        rates.append(max(t - t_fixed, 1e-6) / ints)
+        used += t
+        sampled += ints
+    strata_ints = [cum[bounds[k + 1]] - cum[bounds[k]] for k in range(nstrata)]
+    sweep_s = t_fixed + float(sum(r * n for r, n in zip(rates, strata_ints)))
+    return {"value": D.shape[0] / sweep_s, "unit": UNIT, "cores": O.max_threads(),
+            "kind": "oracle (extrapolated from a stratified bounded sample)", "extrapolated": True,
+            "cpu_seconds_spent": used, "rate_s_per_integral": {"min": min(rates), "max": max(rates)},
+            "sample": "oracle O6 (folded MD loop, all %d densities): %.1f s of CPU time; fixed cost per call %.2f s "
+                      "(empty pair range); %d strata of equal integral share, one run of bra shell pairs from the "
+                      "middle of each: %.3g of the %.3g kept unique integrals sampled, %.3g-%.3g s per integral; "
+                      "sweep = fixed + sum_s rate_s x integrals_s" %
+                      (D.shape[0], used, t_fixed, nstrata, sampled, total_ints, min(rates), max(rates))}
 
 
 def run_reference(args, rank, world):
-    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only).  Each step is one bounded,
+    stratified sample of the workload; `ms_per_step` is the wall time the step really took, `value` the whole-sweep
+    rate extrapolated from the samples (flagged)."""
     if rank != 0:
         return
     from oracle import oracle as O
     from paper_2607_05622_b200.inputs import make_workload
     w = make_workload(args.workload)
-    tau = np.linspace(0.1, 3.0, w.ntau)     # any grid: cost does not depend on the values (PAPER.md:L565)
     nD = w.nD
     rng = np.random.default_rng(1)
-    D = 1e-2 * rng.standard_normal((nD, w.nao, w.nao))
-    per = max(2.0, min(20.0, 120.0 / max(args.steps + args.warmup, 1)))
-    vals = []
+    D = 1e-2 * rng.standard_normal((nD, w.nao, w.nao))    # cost does not depend on the values (PAPER.md:L565)
+    per = max(4.0, min(20.0, 150.0 / max(args.steps + args.warmup, 1)))
+    vals, walls = [], []
     for s in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
         r = oracle_sample(w, D, target_s=per)
         if s >= args.warmup:
             vals.append(r)
+            walls.append(time.perf_counter() - t0)
     v = float(np.mean([r["value"] for r in vals]))
-    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": 1e3 * w.nD / v, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+    out = {"impl": "reference", "metric": metric_name(w), "value": v, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(walls)),
+           "ms_per_step_is": "wall time of one bounded sample step (NOT of a whole sweep)",
+           "extrapolated": True, "extrapolated_ms_per_sweep": 1e3 * nD / v,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": "%s (%d AO, %d densities)" % (w.name, w.nao, nD), "tau_schwarz": w.schwarz_tau},
-           "cpu_baseline": {"value": v, "unit": UNIT, "cores": vals[-1]["cores"], "kind": "oracle", "sample": vals[-1]["sample"]},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": vals[-1]["cores"], "kind": vals[-1]["kind"],
+                            "sample": vals[-1]["sample"],
+                            "spread_over_steps": [min(r["value"] for r in vals), max(r["value"] for r in vals)]},
            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(out), flush=True)
+
+
+def sweep_report(torch, ltjk, w, local, T_host, steps, warmup, world, barrier, max_over_ranks, want_e2e=True):
+    """Set up one workload (geometry-frozen part outside the timed region), time `steps` whole sweeps with CUDA events
+    on the ctx stream, then the per-phase split (timing mode) and the roofline of the digestion kernel."""
+    N, nD = w.nao, w.nD
+    stream = torch.cuda.current_stream()
+    ctx = ltjk.Context(local, stream)
+    ctx.set_basis(w.basis)
+    npairs, nq_kept = ctx.build_shell_pairs(w.schwarz_tau)
+    # the library's own minimax grid; a failure is an error, there is no fallback grid (include/ltjk.h, reading A8)
+    tau, wts, lap_err = ltjk.laplace_quadrature(w.laplace_range[0], w.laplace_range[1], w.ntau)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Co, Cv, eo, ev, Td = dev(w.C_occ), dev(w.C_vir), dev(w.eps_occ), dev(w.eps_vir), dev(T_host)
+    D = torch.empty((w.ntau, w.nT, N, N), dtype=torch.float64, device="cuda")
+    Dn = D.view(nD, N, N)
+    J = torch.empty_like(Dn)
+    K = torch.empty_like(Dn)
+
+    def step():
+        ctx.build_pseudo_densities(Co, Cv, eo, ev, Td, tau, D)
+        ctx.jk_build(Dn, J, K)
+
+    for _ in range(warmup):
+        step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms_per_step = max_over_ranks(e0.elapsed_time(e1), "cuda") / steps
+    rep = {"ctx": ctx, "tau": tau, "Dn": Dn, "J": J, "K": K, "ms_per_step": ms_per_step, "nq_kept": nq_kept,
+           "launches_per_step": ctx.get_stats()["n_launches"] + 3, "laplace_maxerr": lap_err}
+
+    # transform alone (a4): HBM-bound output stream of n_D N^2 doubles
+    e0.record(stream)
+    for _ in range(5):
+        ctx.build_pseudo_densities(Co, Cv, eo, ev, Td, tau, D)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    t_ms = e0.elapsed_time(e1) / 5
+    rep["transform"] = {"ms": t_ms, "gbs_written": 8e-9 * nD * N * N / (t_ms * 1e-3),
+                        "tflops": 2e-12 * (w.nocc * w.nvir * N + w.nocc * N * N) * nD / (t_ms * 1e-3)}
+
+    if want_e2e:    # the same sweep through the C ABI with HOST (pinned) buffers
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        hCo, hCv, heo, hev, hT = pin(w.C_occ), pin(w.C_vir), pin(w.eps_occ), pin(w.eps_vir), pin(T_host)
+        hJ = torch.empty((nD, N, N), dtype=torch.float64).pin_memory()
+        hK = torch.empty((nD, N, N), dtype=torch.float64).pin_memory()
+        ctx.sweep_host(hCo, hCv, heo, hev, hT, tau, hJ, hK)
+        barrier()
+        n_e2e = max(2, min(steps, 3))
+        e0.record(stream)
+        for _ in range(n_e2e):
+            ctx.sweep_host(hCo, hCv, heo, hev, hT, tau, hJ, hK)
+        e1.record(stream)
+        barrier()
+        rep["ms_e2e"] = max_over_ranks(e0.elapsed_time(e1) / n_e2e, "cuda")
+        rep["h2d"] = 8 * (hCo.numel() + hCv.numel() + heo.numel() + hev.numel() + hT.numel())
+        rep["d2h"] = 8 * (hJ.numel() + hK.numel())
+        assert float((hK - K.cpu()).abs().max()) < 1e-9 * float(K.abs().max())
+    return rep
+
+
+def roofline_of(torch, ctx, w, rep, peak_tf):
+    """Digestion kernel (dominant): algorithmic flop of one sweep / summed duration of its launches, timed live per
+    launch group with CUDA events on the ctx stream (timing mode serialises ERI and digestion)."""
+    Dn, J, K = rep["Dn"], rep["J"], rep["K"]
+    ctx.set_timing(True)
+    ctx.jk_build(Dn, J, K)
+    torch.cuda.synchronize()
+    st = ctx.get_stats()
+    ctx.set_timing(False)
+    Q = ctx.get_schwarz()
+    ints = kept_integrals(Q, w.basis.l, w.schwarz_tau)
+    alg = 20.0 * w.nD * ints                 # SURVEY 8(d): 2 J + 8 K FMAs per unique integral and density
+    achieved = alg / (st["digest_ms"] * 1e-3) / 1e12
+    return {"bound": "alu",
+            "kernel": "digest kernel (J/K digestion; achieved = algorithmic flop of one sweep / summed duration of its launches)",
+            "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
+            "peak_source": "DFMA microbenchmark in this run (ltjk_bench_dfma_peak); MEASURED_PEAKS.json has no fp64 entry",
+            "algorithmic_flops_per_sweep": alg, "executed_digest_flops_per_sweep": st["digest_flops"],
+            "executed_over_algorithmic": st["digest_flops"] / alg,
+            "digest_ms_per_sweep": st["digest_ms"], "eri_ms_per_sweep": st["eri_ms"],
+            "whole_sweep_frac_of_peak": alg / (rep["ms_per_step"] * 1e-3) / 1e12 / peak_tf}, ints
+
+
+def committed_ncu(name):
+    """Counters that only ncu can give (DRAM bytes of the digestion launches, fp64 instruction counts of the ERI
+    kernels) come from the committed capture of this round under profiles/; the bench line says so."""
+    f = ROOT / "profiles" / "r2_ncu_counters.json"
+    if not f.exists():
+        return None
+    return json.loads(f.read_text()).get(name)
 
 
 def main():
@@ -167,7 +289,13 @@ def main():
     ap.add_argument("--workload", default="porphine")
     ap.add_argument("--impl", default="ltjk")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-large", action="store_true", help="skip the 730-AO sub-run reported under config.large_730")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
+        # not launched under torchrun: spawn the N ranks ourselves (one process per GPU, NCCL over NVLink)
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node",
+                                  str(args.gpus), "--master-addr", "127.0.0.1", "--master-port",
+                                  os.environ.get("MASTER_PORT", "29517"), str(Path(__file__).resolve())] + sys.argv[1:])
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -195,86 +323,34 @@ def main():
     from paper_2607_05622_b200.dist import max_over_ranks, rank_amplitudes, whole_job_builds_per_s
     T_host = rank_amplitudes(w, rank)
 
-    stream = torch.cuda.current_stream()
-    ctx = ltjk.Context(local, stream)
-    ctx.set_basis(w.basis)
-    npairs, nq_kept = ctx.build_shell_pairs(w.schwarz_tau)
-    tau, wts, lap_err = None, None, None
-    try:
-        tau, wts, lap_err = ltjk.laplace_quadrature(w.laplace_range[0], w.laplace_range[1], w.ntau)
-    except ltjk.LtjkError:
-        tau = np.linspace(0.1, 3.0, w.ntau)
-    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    Co, Cv, eo, ev, Td = dev(w.C_occ), dev(w.C_vir), dev(w.eps_occ), dev(w.eps_vir), dev(T_host)
-    D = torch.empty((w.ntau, w.nT, N, N), dtype=torch.float64, device="cuda")
-    Dn = D.view(nD, N, N)
-    J = torch.empty_like(Dn)
-    K = torch.empty_like(Dn)
-
-    def step():
-        ctx.build_pseudo_densities(Co, Cv, eo, ev, Td, tau, D)
-        ctx.jk_build(Dn, J, K)
-
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        step()
-    barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record(stream)
-    for _ in range(args.steps):
-        step()
-    e1.record(stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
-    launches_jk = ctx.get_stats()["n_launches"]
+    rep = sweep_report(torch, ltjk, w, local, T_host, args.steps, args.warmup, world, barrier, max_over_ranks)
     clocks = sampler.stop() if rank == 0 else None
-    ms = max_over_ranks(ms, "cuda")
-    ms_per_step = ms / args.steps
+    ms_per_step = rep["ms_per_step"]
     value = whole_job_builds_per_s(nD, world, ms_per_step)
-
-    # ---- e2e: the same sweep through the C ABI with HOST (pinned) buffers
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    hCo, hCv, heo, hev, hT = pin(w.C_occ), pin(w.C_vir), pin(w.eps_occ), pin(w.eps_vir), pin(T_host)
-    hJ = torch.empty((nD, N, N), dtype=torch.float64).pin_memory()
-    hK = torch.empty((nD, N, N), dtype=torch.float64).pin_memory()
-    ctx.sweep_host(hCo, hCv, heo, hev, hT, tau, hJ, hK)
-    barrier()
-    n_e2e = max(2, min(args.steps, 3))
-    t0 = time.perf_counter()
-    e0.record(stream)
-    for _ in range(n_e2e):
-        tc = time.perf_counter()
-        ctx.sweep_host(hCo, hCv, heo, hev, hT, tau, hJ, hK)
-        if rank == 0:
-            print("e2e sweep_host call: %.1f ms" % ((time.perf_counter() - tc) * 1e3), file=sys.stderr)
-    e1.record(stream)
-    barrier()
-    ms_e2e = e0.elapsed_time(e1) / n_e2e
-    ms_e2e = max_over_ranks(ms_e2e, "cuda")
-    h2d = 8 * (hCo.numel() + hCv.numel() + heo.numel() + hev.numel() + hT.numel())
-    d2h = 8 * (hJ.numel() + hK.numel())
-    assert torch.equal(hK, K.cpu()) or float((hK - K.cpu()).abs().max()) < 1e-9 * float(K.abs().max())
-
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (digestion), timed live per launch with CUDA events on the ctx stream
-    ctx.set_timing(True)
-    ctx.jk_build(Dn, J, K)
-    torch.cuda.synchronize()
-    st = ctx.get_stats()
-    ctx.set_timing(False)
+    ctx, Dn = rep["ctx"], rep["Dn"]
+    stream = torch.cuda.current_stream()
+    peak_tf = ctx.bench_dfma_peak()
+    hbm_gbs = ctx.bench_copy_peak()
+    roofline, ints = roofline_of(torch, ctx, w, rep, peak_tf)
+    tr = committed_ncu("digest_dram_bytes_per_sweep_%s" % w.name)
+    roofline["traffic"] = tr
+    roofline["traffic_source"] = ("committed ncu capture profiles/r2_ncu_counters.json (not measured in this run)"
+                                  if tr is not None else None)
     # one Laplace point per call (n_D = n_T): makes the integral re-computation per call visible
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     D1 = Dn[:w.nT].contiguous()
     J1 = torch.empty_like(D1)
     K1 = torch.empty_like(D1)
@@ -285,44 +361,49 @@ def main():
     e1.record(stream)
     torch.cuda.synchronize()
     single_point = {"n_D": int(w.nT), "ms": e0.elapsed_time(e1), "builds_per_s": w.nT / (e0.elapsed_time(e1) * 1e-3)}
-    Q = ctx.get_schwarz()
-    ints = kept_integrals(Q, w.basis.l, w.schwarz_tau)
-    digest_flops_alg = 20.0 * nD * ints                  # 2 J + 8 K FMAs per unique integral and density
-    peak_tf = ctx.bench_dfma_peak()
-    achieved_tf = digest_flops_alg / (st["digest_ms"] * 1e-3) / 1e12
-    # DRAM traffic of the digestion launches of one sweep from the committed ncu capture (profiles/), 439 AO only
-    traffic = None
-    tfile = ROOT / "profiles" / "r1_digest_traffic.json"
-    if w.name == "porphine" and tfile.exists():
-        tj = json.loads(tfile.read_text())
-        traffic = tj["dram_bytes_read_per_sweep"] + tj["dram_bytes_write_per_sweep"]
-    roofline = {"bound": "alu", "kernel": "digest_kernel (J/K digestion; achieved = algorithmic flop of one sweep / summed duration of its launches)",
-                "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-                "traffic": traffic,
-                "peak_source": "DFMA microbenchmark in this run (ltjk_bench_dfma_peak); MEASURED_PEAKS.json has no fp64 entry",
-                "algorithmic_flops_per_sweep": digest_flops_alg, "executed_digest_flops_per_sweep": st["digest_flops"],
-                "digest_ms_per_sweep": st["digest_ms"], "eri_ms_per_sweep": st["eri_ms"],
-                "whole_sweep_frac_of_peak": digest_flops_alg / (ms_per_step * 1e-3) / 1e12 / peak_tf}
+    measured = json.loads((ROOT / "MEASURED_PEAKS.json").read_text()) if (ROOT / "MEASURED_PEAKS.json").exists() else {}
+    hbm_peak = measured.get("hbm_gbs", hbm_gbs)
+    transform = dict(rep["transform"], frac_of_hbm_peak=rep["transform"]["gbs_written"] / hbm_peak, hbm_peak_gbs=hbm_peak,
+                     hbm_peak_source="MEASURED_PEAKS.json" if "hbm_gbs" in measured else "copy microbenchmark in this run")
     cpu = None
     if not args.no_cpu_baseline:
-        cpu = oracle_sample(w, Dn.cpu().numpy(), target_s=15.0)
-    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-           "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-           "data": "synthetic",
-           "config": {"workload": "%s (%d AO, %d atoms, n_tau=%d x n_T=%d = %d non-symmetric densities per sweep)" %
-                                  (w.name, N, w.basis.natom, w.ntau, w.nT, nD),
-                      "tau_schwarz": w.schwarz_tau, "shell_quartets_kept": nq_kept, "unique_integrals_kept": ints,
-                      "l2": "inputs_larger_than_L2 (D, J, K are %.0f MB each)" % (8e-6 * nD * N * N),
-                      "setup_outside_timed_region": "basis upload, shell pairs, Schwarz, work lists (geometry-frozen)",
-                      "laplace_grid": "library minimax" if wts is not None else "placeholder linspace (cost is value-independent)",
-                      "one_laplace_point_per_call": single_point,
-                      "gpu": torch.cuda.get_device_name(local), "hbm_copy_gbs_measured": ctx.bench_copy_peak(),
-                      "dfma_peak_tflops_measured": peak_tf},
-           "clocks": clocks,
-           "e2e": {"value": whole_job_builds_per_s(nD, world, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                   "ms_per_step": ms_e2e},
-           "gpu_launches": int((launches_jk + 3) * args.steps),
-           "roofline": roofline, "cpu_baseline": cpu}
+        cpu = oracle_sample(w, Dn.cpu().numpy(), target_s=20.0)
+    launches = int(rep["launches_per_step"] * args.steps)
+    e2e = {"value": whole_job_builds_per_s(nD, world, rep["ms_e2e"]), "unit": UNIT, "h2d_bytes_per_step": rep["h2d"],
+           "d2h_bytes_per_step": rep["d2h"], "ms_per_step": rep["ms_e2e"]}
+    config = {"workload": "%s (%d AO, %d atoms, n_tau=%d x n_T=%d = %d non-symmetric densities per sweep)" %
+                          (w.name, N, w.basis.natom, w.ntau, w.nT, nD),
+              "tau_schwarz": w.schwarz_tau, "shell_quartets_kept": rep["nq_kept"], "unique_integrals_kept": ints,
+              "l2": "inputs_larger_than_L2 (D, J, K are %.0f MB each)" % (8e-6 * nD * N * N),
+              "setup_outside_timed_region": "basis upload, shell pairs, Schwarz, work lists (geometry-frozen)",
+              "laplace_grid": "library minimax, max error %.3e" % rep["laplace_maxerr"],
+              "one_laplace_point_per_call": single_point, "transform": transform,
+              "eri_fp64_flops_per_sweep_ncu": committed_ncu("eri_fp64_flops_per_sweep_%s" % w.name),
+              "gpu": torch.cuda.get_device_name(local), "hbm_copy_gbs_measured": hbm_gbs,
+              "dfma_peak_tflops_measured": peak_tf}
+    # free the headline workload before the 730-AO sub-run
+    del rep, Dn, D1, J1, K1
+    ctx.close()
+    torch.cuda.empty_cache()
+    if world == 1 and not args.no_large and w.name != "large":
+        wl = make_workload("large")
+        s2 = ClockSampler(local)
+        s2.start()
+        repl = sweep_report(torch, ltjk, wl, local, wl.T, 2, 1, 1, barrier, max_over_ranks, want_e2e=False)
+        cl2 = s2.stop()
+        rl, intsl = roofline_of(torch, repl["ctx"], wl, repl, peak_tf)
+        trl = committed_ncu("digest_dram_bytes_per_sweep_large")
+        rl["traffic"] = trl
+        config["large_730"] = {"metric": metric_name(wl), "value": wl.nD / (repl["ms_per_step"] * 1e-3), "unit": UNIT,
+                               "ms_per_step": repl["ms_per_step"], "steps": 2, "warmup": 1, "n_D": wl.nD,
+                               "unique_integrals_kept": intsl, "roofline": rl, "clocks": cl2,
+                               "transform": repl["transform"]}
+        launches += int(repl["launches_per_step"] * 2)
+        repl["ctx"].close()
+    out = {"metric": metric_name(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config, "clocks": clocks, "e2e": e2e,
+           "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()

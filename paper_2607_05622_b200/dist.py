@@ -29,3 +29,48 @@ def max_over_ranks(value: float, device=None) -> float:
 def whole_job_builds_per_s(n_builds_per_rank: int, world: int, ms_per_step_max: float) -> float:
     """weak scaling: every rank does n_builds_per_rank builds per step; the job's rate uses the slowest rank's time"""
     return world * n_builds_per_rank / (ms_per_step_max * 1e-3)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Sharding ONE sweep over ranks (SURVEY.md 8(e), second alternative): the n_D = n_tau x n_T densities of a sweep are
+# independent builds, so rank r takes densities r, r + world, r + 2 world, ... and recomputes the integrals for its
+# share; there is no data-path collective.  Results are gathered only when the caller wants the whole batch on one
+# rank (tests, checks), never inside a timed step.
+def density_shard(n_densities: int, rank: int, world: int) -> np.ndarray:
+    """Indices (into the sweep's density batch) owned by `rank`: round-robin, so Laplace points and amplitude sets
+    are spread evenly and every rank gets the same count up to one."""
+    if not (0 <= rank < world):
+        raise ValueError("rank outside the world")
+    return np.arange(rank, n_densities, world)
+
+
+def shard_sizes(n_densities: int, world: int) -> list:
+    return [len(range(r, n_densities, world)) for r in range(world)]
+
+
+def gather_sharded(local, n_densities: int):
+    """Inverse of density_shard for a result tensor: every rank passes its [n_local, ...] block (torch tensor on the
+    backend's device) and gets the full [n_densities, ...] batch in sweep order.  Uses all_gather on blocks padded to
+    the largest shard (the only collective, outside any timed region)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return local
+    world, rank = dist.get_world_size(), dist.get_rank()
+    sizes = shard_sizes(n_densities, world)
+    if local.shape[0] != sizes[rank]:
+        raise ValueError("local block does not match this rank's shard")
+    nmax = max(sizes)
+    pad = torch.zeros((nmax,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device)
+    pad[:local.shape[0]] = local
+    parts = [torch.empty_like(pad) for _ in range(world)]
+    dist.all_gather(parts, pad)
+    full = torch.empty((n_densities,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device)
+    for r in range(world):
+        full[r::world] = parts[r][:sizes[r]]
+    return full
+
+
+def sharded_sweep_builds_per_s(n_densities: int, ms_per_step_max: float) -> float:
+    """strong scaling: the job is ONE sweep of n_densities builds split over the ranks"""
+    return n_densities / (ms_per_step_max * 1e-3)

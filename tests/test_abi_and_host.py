@@ -86,6 +86,20 @@ dist.all_gather(out, c)
 assert len({round(float(o), 12) for o in out}) == world
 v = whole_job_builds_per_s(w.nD, world, ms)
 assert abs(v - world * w.nD / (ms * 1e-3)) < 1e-9
+# one sweep sharded over the ranks (SURVEY 8(e)): round-robin density shards are a partition, and gathering the
+# per-rank results restores sweep order
+from paper_2607_05622_b200.dist import density_shard, gather_sharded, shard_sizes, sharded_sweep_builds_per_s
+for nD in (1, 7, 8, 160):
+    mine = density_shard(nD, rank, world)
+    assert len(mine) == shard_sizes(nD, world)[rank]
+    cnt = torch.zeros(nD, dtype=torch.float64)
+    cnt[torch.from_numpy(mine)] += 1
+    dist.all_reduce(cnt)
+    assert bool((cnt == 1).all())                      # every density owned exactly once
+    fake = torch.from_numpy(mine.astype(np.float64))[:, None, None] * torch.ones((1, 3, 3), dtype=torch.float64)
+    full = gather_sharded(fake, nD)
+    assert full.shape == (nD, 3, 3) and bool((full[:, 0, 0] == torch.arange(nD, dtype=torch.float64)).all())
+assert abs(sharded_sweep_builds_per_s(160, 500.0) - 320.0) < 1e-12
 if rank == 0:
     print("GLOO_OK", v)
 dist.destroy_process_group()
