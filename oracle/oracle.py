@@ -327,3 +327,32 @@ def laplace_accumulate(tau, w, omega: float, X: np.ndarray) -> np.ndarray:
     for a in range(X.shape[0]):
         out += w[a] * np.exp(omega * tau[a]) * X[a]        # w~_a(omega) = w_a e^{omega tau_a}, Eq. (21)
     return out
+
+
+# ---------------------------------------------------------------------------------------------------------
+# SURVEY 8(f) N3.  Particle-particle ladder (Algorithm 2):
+#     L[p, a, b] = sum_{ef} (ae|bf) X[p, e, f],        p = a compound occupied pair index (ij),
+# with (ae|bf) the integrals over the virtual orbitals C_vir, written as the definition: the AO tensor of O7
+# transformed to the virtual MO basis (a library contraction as the step), then the explicit sum over (e, f).
+def pp_ladder(eri: np.ndarray, C_vir: np.ndarray, X: np.ndarray) -> np.ndarray:
+    mo = np.einsum("mnkr,ma,ne,kb,rf->aebf", eri, C_vir, C_vir, C_vir, C_vir, optimize=True)   # (ae|bf)
+    return np.einsum("aebf,pef->pab", mo, X, optimize=True)
+
+
+def pp_ladder_loops(eri: np.ndarray, C_vir: np.ndarray, X: np.ndarray) -> np.ndarray:
+    """The same sum as explicit loops over every index (tiny cases only; pins the einsum index strings)."""
+    n, nv = C_vir.shape
+    L = np.zeros((X.shape[0], nv, nv))
+    for a in range(nv):
+        for b in range(nv):
+            for e in range(nv):
+                for f in range(nv):
+                    g = 0.0                                   # (ae|bf) = sum C_ma C_ne (mn|kr) C_kb C_rf
+                    for m in range(n):
+                        for nn in range(n):
+                            for k in range(n):
+                                for r in range(n):
+                                    g += C_vir[m, a] * C_vir[nn, e] * eri[m, nn, k, r] * C_vir[k, b] * C_vir[r, f]
+                    for p in range(X.shape[0]):
+                        L[p, a, b] += g * X[p, e, f]
+    return L
