@@ -184,12 +184,13 @@ def run_reference(args, rank, world):
     print(json.dumps(out), flush=True)
 
 
-def sweep_report(torch, ltjk, w, local, T_host, steps, warmup, world, barrier, max_over_ranks, want_e2e=True):
+def sweep_report(torch, ltjk, w, local, T_host, steps, warmup, world, barrier, max_over_ranks, want_e2e=True, mode=0):
     """Set up one workload (geometry-frozen part outside the timed region), time `steps` whole sweeps with CUDA events
     on the ctx stream, then the per-phase split (timing mode) and the roofline of the digestion kernel."""
     N, nD = w.nao, w.nD
     stream = torch.cuda.current_stream()
     ctx = ltjk.Context(local, stream)
+    ctx.set_digest_mode(mode)
     ctx.set_basis(w.basis)
     npairs, nq_kept = ctx.build_shell_pairs(w.schwarz_tau)
     # the library's own minimax grid; a failure is an error, there is no fallback grid (include/ltjk.h, reading A8)
@@ -217,7 +218,8 @@ def sweep_report(torch, ltjk, w, local, T_host, steps, warmup, world, barrier, m
     barrier()
     ms_per_step = max_over_ranks(e0.elapsed_time(e1), "cuda") / steps
     rep = {"ctx": ctx, "tau": tau, "Dn": Dn, "J": J, "K": K, "ms_per_step": ms_per_step, "nq_kept": nq_kept,
-           "launches_per_step": ctx.get_stats()["n_launches"] + 3, "laplace_maxerr": lap_err}
+           "launches_per_step": ctx.get_stats()["n_launches"] + 3, "laplace_maxerr": lap_err,
+           "digest_mode": ctx.get_digest_mode()}
 
     # transform alone (a4): HBM-bound output stream of n_D N^2 doubles
     e0.record(stream)
@@ -289,6 +291,7 @@ def main():
     ap.add_argument("--workload", default="porphine")
     ap.add_argument("--impl", default="ltjk")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", type=int, default=0, help="digestion strategy (ltjk_set_digest_mode): 0 auto, 1 panels, 2 pair lists")
     ap.add_argument("--no-large", action="store_true", help="skip the 730-AO sub-run reported under config.large_730")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
@@ -331,7 +334,7 @@ def main():
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    rep = sweep_report(torch, ltjk, w, local, T_host, args.steps, args.warmup, world, barrier, max_over_ranks)
+    rep = sweep_report(torch, ltjk, w, local, T_host, args.steps, args.warmup, world, barrier, max_over_ranks, mode=args.mode)
     clocks = sampler.stop() if rank == 0 else None
     ms_per_step = rep["ms_per_step"]
     value = whole_job_builds_per_s(nD, world, ms_per_step)
@@ -377,6 +380,7 @@ def main():
               "l2": "inputs_larger_than_L2 (D, J, K are %.0f MB each)" % (8e-6 * nD * N * N),
               "setup_outside_timed_region": "basis upload, shell pairs, Schwarz, work lists (geometry-frozen)",
               "laplace_grid": "library minimax, max error %.3e" % rep["laplace_maxerr"],
+              "digest_mode": {1: "block panels", 2: "pair lists"}[rep["digest_mode"]],
               "one_laplace_point_per_call": single_point, "transform": transform,
               "eri_fp64_flops_per_sweep_ncu": committed_ncu("eri_fp64_flops_per_sweep_%s" % w.name),
               "gpu": torch.cuda.get_device_name(local), "hbm_copy_gbs_measured": hbm_gbs,
@@ -389,7 +393,7 @@ def main():
         wl = make_workload("large")
         s2 = ClockSampler(local)
         s2.start()
-        repl = sweep_report(torch, ltjk, wl, local, wl.T, 2, 1, 1, barrier, max_over_ranks, want_e2e=False)
+        repl = sweep_report(torch, ltjk, wl, local, wl.T, 2, 1, 1, barrier, max_over_ranks, want_e2e=False, mode=args.mode)
         cl2 = s2.stop()
         rl, intsl = roofline_of(torch, repl["ctx"], wl, repl, peak_tf)
         trl = committed_ncu("digest_dram_bytes_per_sweep_large")
@@ -397,6 +401,7 @@ def main():
         config["large_730"] = {"metric": metric_name(wl), "value": wl.nD / (repl["ms_per_step"] * 1e-3), "unit": UNIT,
                                "ms_per_step": repl["ms_per_step"], "steps": 2, "warmup": 1, "n_D": wl.nD,
                                "unique_integrals_kept": intsl, "roofline": rl, "clocks": cl2,
+                               "digest_mode": {1: "block panels", 2: "pair lists"}[repl["digest_mode"]],
                                "transform": repl["transform"]}
         launches += int(repl["launches_per_step"] * 2)
         repl["ctx"].close()

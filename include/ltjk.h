@@ -122,6 +122,15 @@ int ltjk_laplace_fock(ltjk_ctx* ctx, int nD, const double* J, const double* K, i
 int ltjk_laplace_accumulate(ltjk_ctx* ctx, int ntau, int nT, long long nelem, const double* tau_host,
                             const double* w_host, double omega, const double* X, double* Y);
 
+/* AO-direct particle-particle ladder (Algorithm 2; L432-434)
+ *     L[p][a][b] = sum_{e,f} (ae|bf) X[p][e][f],      p = 0..npair-1 a compound occupied-pair index (ij),
+ * with (ae|bf) the integrals over the virtual orbitals C_vir [N][nvir], never formed: every X_p is turned into the
+ * non-symmetric AO density C_vir X_p C_vir^T, the batch goes through the K-only path of ltjk_jk_build in chunks of
+ * `chunk` densities (0 = default 160), and K is transformed back, L_p = C_vir^T K[D_p] C_vir.  No prefactors.
+ * C_vir, X [npair][nvir][nvir], L [npair][nvir][nvir] are DEVICE pointers, row-major; L is overwritten.  Work is
+ * enqueued on the ctx stream; scratch of 2 * chunk * N^2 doubles is taken from the stream-ordered pool. */
+int ltjk_pp_ladder(ltjk_ctx* ctx, int nvir, const double* C_vir, int npair, const double* X, double* L, int chunk);
+
 /* Statistics of the last ltjk_jk_build on this context (HOST outputs, any may be NULL):
  *   n_launches    kernels launched
  *   eri_quartets  contracted shell quartets evaluated (4-fold unique: A>=B, C>=D, all bra x ket)
@@ -130,6 +139,19 @@ int ltjk_laplace_accumulate(ltjk_ctx* ctx, int ntau, int nT, long long nelem, co
 int ltjk_get_stats(const ltjk_ctx* ctx, long long* n_launches, long long* eri_quartets, double* digest_flops,
                    double* eri_ms, double* digest_ms);
 int ltjk_set_timing(ltjk_ctx* ctx, int enable);
+
+/* Digestion strategy for step a8, read by the NEXT ltjk_build_shell_pairs ("once Schwarz screening is
+ * applied"; L320-322 Eq. 25):
+ *   1  block panels: dense integral panels of l-homogeneous AO blocks, six GEMM views; best when nearly all
+ *      quartets inside the surviving block pairs pass the Schwarz test (compact molecules);
+ *   2  pair lists: Q-sorted partner lists with staircase cut-offs, screened quartets are neither stored nor
+ *      multiplied; best for extended molecules;
+ *   0  automatic (default): mode 2 when fewer than half of all canonical shell quartets pass the Schwarz test,
+ *      mode 1 otherwise.
+ * Results are the same sums up to rounding order.  Returns LTJK_EINVAL for other values. */
+int ltjk_set_digest_mode(ltjk_ctx* ctx, int mode);
+/* The strategy (1 or 2) chosen by the last ltjk_build_shell_pairs; LTJK_ENOBASIS before it. */
+int ltjk_get_digest_mode(const ltjk_ctx* ctx, int* mode);
 
 /* Test hook: contracted Cartesian shell quartet (A B|C D) in the caller's shell indices, evaluated by the
  * device ERI kernel, written to HOST out[na*nb*nc*nd] (row-major a,b,c,d).  Synchronises. */

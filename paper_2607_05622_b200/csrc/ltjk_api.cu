@@ -32,6 +32,7 @@ void free_tables(ltjk_ctx* c)
     t.boys = boys;
     c->d_items = nullptr; c->d_subs = nullptr; c->d_chunkmask = nullptr; c->n_maskbits = 0; c->d_panel = nullptr; c->panel_cap = 0; c->panel_half = 0; c->n_items = 0;
     c->have_pairs = false;
+    free_pairlists(c);
 }
 
 void free_work(ltjk_ctx* c)

@@ -99,6 +99,17 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
         c->n_quartets_kept = (ordered + diag) / 2;
     }
 
+    // ---- digestion strategy (include/ltjk.h: ltjk_set_digest_mode).  Automatic: pair lists when fewer than half of the
+    // canonical shell quartets survive the Schwarz test (extended molecules: the dense block panels would be mostly
+    // zeros), block panels otherwise.
+    {
+        const double npairs_all = 0.5 * (double)ns * (ns + 1);
+        const double kept_frac = (double)c->n_quartets_kept / (0.5 * npairs_all * (npairs_all + 1.0));
+        c->digest_mode = c->digest_mode_req ? c->digest_mode_req : (kept_frac < 0.5 ? 2 : 1);
+    }
+    const bool panels = (c->digest_mode == 1);
+    c->subs.clear(); c->groups.clear();
+
     // ---- block pairs ranked class-major, panel offsets
     const int nblk = t.nblk;
     c->pair_I.clear(); c->pair_J.clear();
@@ -142,10 +153,11 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     long long total = c->koff[npair] * c->koff[npair];      // never need more than everything at once
     c->panel_half = std::max<long long>(std::min<long long>(bytes / 16, total), maxpanel);
     c->panel_cap = 2 * c->panel_half;
-    LTJK_CUDA(c, cudaMalloc(&c->d_panel, sizeof(double) * c->panel_cap));
-
     std::vector<DigestItem> items;
-    build_work(c, items);
+    if (panels) {
+        LTJK_CUDA(c, cudaMalloc(&c->d_panel, sizeof(double) * c->panel_cap));
+        build_work(c, items);
+    }
     c->n_items = (long long)items.size();
     {   // chunk mask layout: partner items of one tile share nothing here; one bit per (item, chunk)
         unsigned long long bits = 0;
@@ -169,9 +181,12 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
         (rc = upload(c, &t.koff, c->koff)) || (rc = upload(c, &t.rank_of, c->rank_of)) ||
         (rc = upload(c, &t.ao_perm, c->ao_perm)) || (rc = upload(c, &t.ao_sh, ao_sh)))
         return rc;
-    LTJK_CUDA(c, cudaMalloc(&c->d_chunkmask, (size_t)c->n_maskbits + 16));
-    if ((rc = launch_chunk_mask(c))) return rc;
+    if (panels) {
+        LTJK_CUDA(c, cudaMalloc(&c->d_chunkmask, (size_t)c->n_maskbits + 16));
+        if ((rc = launch_chunk_mask(c))) return rc;
+    }
     LTJK_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (!panels && (rc = build_pairlists(c))) return rc;
     c->have_pairs = true;
     if (n_pairs) *n_pairs = (long long)ns * (ns + 1) / 2;
     if (n_quartets_kept) *n_quartets_kept = c->n_quartets_kept;
@@ -196,7 +211,7 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
     if (nD <= 0 || !D || (!J && !K)) return set_err(c, LTJK_EINVAL, "jk_build: bad arguments");
     cudaSetDevice(c->device);
     int TN, nb;
-    digest_colblocks(nD, &TN, &nb);
+    digest_colblocks(nD, c->digest_mode, &TN, &nb);
     const int nDp = TN * nb * 32;
     int rc;
     if ((rc = ensure_work(c, nDp))) return rc;
@@ -208,6 +223,44 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
     if (K) LTJK_CUDA(c, cudaMemsetAsync(c->Kt, 0, wbytes, c->stream));
     cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
     if (c->timing) { cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventCreate(&e2); }
+    if (c->digest_mode == 2) {
+        // pair-list pipeline: per chunk, clear its ring half, generate the integrals of the chunk under all role
+        // assignments (eri_stream), digest them (ctx stream); chunk c+1 is generated while chunk c is digested
+        c->eri_stream = c->timing ? c->stream : c->own_stream;
+        if (!c->timing) {
+            LTJK_CUDA(c, cudaEventRecord(c->ev_start, c->stream));
+            LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_start, 0));
+        }
+        long long gi = 0;
+        c->pcounter_next = 0;
+        LTJK_CUDA(c, cudaMemsetAsync(c->d_pcounter, 0, sizeof(int) * c->pcounter_cap, c->stream));
+        for (const PChunk& ch : c->pchunks) {
+            if (!c->timing && gi >= 2) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[ch.buf], 0));
+            if (c->timing) cudaEventRecord(e0, c->stream);
+            if ((rc = launch_pzero(c, ch))) return rc;
+            if ((rc = launch_peri_chunk(c, ch))) return rc;
+            if (c->timing) cudaEventRecord(e1, c->stream);
+            else {
+                LTJK_CUDA(c, cudaEventRecord(c->ev_eri[ch.buf], c->eri_stream));
+                LTJK_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_eri[ch.buf], 0));
+            }
+            if ((rc = launch_pdigest(c, ch, nDp, J != nullptr, K != nullptr))) return rc;
+            if (!c->timing) LTJK_CUDA(c, cudaEventRecord(c->ev_dig[ch.buf], c->stream));
+            ++gi;
+            if (c->timing) {
+                cudaEventRecord(e2, c->stream);
+                cudaEventSynchronize(e2);
+                float a = 0.f, b = 0.f;
+                cudaEventElapsedTime(&a, e0, e1); cudaEventElapsedTime(&b, e1, e2);
+                c->st_eri_ms += a; c->st_digest_ms += b;
+            }
+            c->st_digest_flops += 2.0 * nDp * ((J ? ch.exec_rows_chunks_J : 0.0) + (K ? ch.exec_rows_chunks_K : 0.0));
+        }
+        c->st_quartets = c->n_quartets_kept;
+        if (c->timing) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2); }
+        if ((rc = launch_unpack_results(c, nD, nDp, J, K))) return rc;
+        return LTJK_OK;
+    }
 
     // Two-stream pipeline over the two halves of the panel ring: ERI(g+1) on eri_stream overlaps digest(g) on
     // the context stream (both are DFMA-bound; the overlap fills launch tails and hides the long single-thread
@@ -334,6 +387,41 @@ int ltjk_laplace_fock(ltjk_ctx* c, int nD, const double* J, const double* K, int
     return launch_laplace_fock(c, nD, J, K, nmo, C, F);
 }
 
+int ltjk_pp_ladder(ltjk_ctx* c, int nvir, const double* C_vir, int npair, const double* X, double* L, int chunk)
+{
+    if (!c) return LTJK_EINVAL;
+    if (!c->have_pairs) return set_err(c, LTJK_ENOBASIS, "pp_ladder: shell pairs not built");
+    if (nvir <= 0 || npair <= 0 || chunk < 0 || !C_vir || !X || !L) return set_err(c, LTJK_EINVAL, "pp_ladder: bad arguments");
+    cudaSetDevice(c->device);
+    // column chunks of the compound pair index ("column-chunked over the o^2 trial columns at peak
+    // device memory O(chunk n_ao^2)"); the default is the batch size the digestion kernels are tuned for
+    if (chunk == 0) chunk = 160;
+    chunk = std::min(chunk, npair);
+    const long long N = c->nao;
+    double *D = nullptr, *K = nullptr, *zero = nullptr;
+    LTJK_CUDA(c, cudaMallocAsync(&D, sizeof(double) * (size_t)chunk * N * N, c->stream));
+    LTJK_CUDA(c, cudaMallocAsync(&K, sizeof(double) * (size_t)chunk * N * N, c->stream));
+    LTJK_CUDA(c, cudaMallocAsync(&zero, sizeof(double) * nvir, c->stream));
+    LTJK_CUDA(c, cudaMemsetAsync(zero, 0, sizeof(double) * nvir, c->stream));
+    const double tau0 = 0.0;
+    int rc = LTJK_OK;
+    long long launches = 0, quartets = 0;
+    double flops = 0.0;
+    for (int p0 = 0; p0 < npair && !rc; p0 += chunk) {
+        const int n = std::min(chunk, npair - p0);
+        const double* Xc = X + (size_t)p0 * nvir * nvir;
+        // D_p = C_v X_p C_v^T: the pseudo-density transform at tau = 0 with both coefficient blocks = C_vir
+        rc = launch_pseudo_densities(c, nvir, nvir, C_vir, C_vir, zero, zero, n, Xc, 1, &tau0, D);
+        if (!rc) rc = ltjk_jk_build(c, n, D, nullptr, K);                       // K-only fast path
+        launches += c->st_launches + 3; quartets += c->st_quartets; flops += c->st_digest_flops;
+        if (!rc) rc = launch_mo_transform(c, n, K, 1.0, nullptr, 0.0, nvir, C_vir, L + (size_t)p0 * nvir * nvir);
+        launches += 3;
+    }
+    c->st_launches = launches; c->st_quartets = quartets; c->st_digest_flops = flops;
+    cudaFreeAsync(D, c->stream); cudaFreeAsync(K, c->stream); cudaFreeAsync(zero, c->stream);
+    return rc;
+}
+
 int ltjk_laplace_accumulate(ltjk_ctx* c, int ntau, int nT, long long nelem, const double* tau_host,
                             const double* w_host, double omega, const double* X, double* Y)
 {
@@ -353,6 +441,21 @@ int ltjk_get_stats(const ltjk_ctx* c, long long* n_launches, long long* eri_quar
     if (digest_flops) *digest_flops = c->st_digest_flops;
     if (eri_ms) *eri_ms = c->st_eri_ms;
     if (digest_ms) *digest_ms = c->st_digest_ms;
+    return LTJK_OK;
+}
+
+int ltjk_set_digest_mode(ltjk_ctx* c, int mode)
+{
+    if (!c || mode < 0 || mode > 2) return LTJK_EINVAL;
+    c->digest_mode_req = mode;
+    return LTJK_OK;
+}
+
+int ltjk_get_digest_mode(const ltjk_ctx* c, int* mode)
+{
+    if (!c || !mode) return LTJK_EINVAL;
+    if (!c->have_pairs) return LTJK_ENOBASIS;
+    *mode = c->digest_mode;
     return LTJK_OK;
 }
 

@@ -15,16 +15,13 @@
 // One CTA owns a 128-row tile of one output block for all (<= 192) densities, keeps it in registers over a RUN of
 // panels sharing that output block, and flushes once with coalesced fp64 reductions.
 #include "ltjk_internal.h"
+#include "digest_common.h"
 #include <cstdio>
+#include <cstdlib>
 #include <algorithm>
 
 namespace ltjk {
 
-constexpr int kMT = kDigestRows;   // rows per CTA (128)
-constexpr int kMTP = kMT + 2;      // padded row stride of the A tile in shared memory
-constexpr int kKC = 16;            // contraction chunk
-constexpr int kStages = 5;
-constexpr int kTM = 16;            // rows per consumer thread
 constexpr int kMaxNC = 1024;   // max columns of one panel view (block AO count squared)
 
 struct DigestArgs {
@@ -40,47 +37,6 @@ struct DigestArgs {
     int nDp;
 };
 
-__device__ __forceinline__ void cp_async8(void* smem, const void* gmem, bool valid)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    const int sz = valid ? 8 : 0;
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
-}
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool valid)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    const int sz = valid ? 16 : 0;
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
-
-// ---- mbarrier helpers (producer/consumer pipeline inside one CTA) -------------------------------------------------
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_arrive(unsigned long long* bar)
-{
-    asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar))
-                 : "memory");
-}
-// arrive on `bar` once all cp.async issued so far by this thread have landed (the count was provisioned at init)
-__device__ __forceinline__ void mbar_arrive_on_cp_async(unsigned long long* bar)
-{
-    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"((unsigned)__cvta_generic_to_shared(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
-{
-    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
-    asm volatile(
-        "{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(a),
-        "r"(parity)
-        : "memory");
-}
-
 template <int TN>
 struct DigestSmem {
     double A[kStages][kKC][kMTP];
@@ -93,11 +49,6 @@ struct DigestSmem {
     unsigned bcol[kMaxNC];
 };
 
-constexpr int kConsumerWarps = 8;
-constexpr int kProducerWarps = 4;
-constexpr int kProducerThreads = kProducerWarps * 32;
-constexpr int kDigestThreads = (kConsumerWarps + kProducerWarps) * 32;
-static_assert(kConsumerWarps * kTM == kMT, "consumer warps must cover the row tile");
 
 // Warp-specialised, persistent, one CTA per SM: warps 0..7 (two warpgroups) are consumers -- LDS + DFMA only, thread
 // tile 16 x TN, warp w owns rows 16w..16w+15 and all 32 TN columns -- and warps 8..11 (one warpgroup) are producers:
@@ -396,11 +347,17 @@ static int launch_digest_tn(ltjk_ctx* c, const DigestArgs& g, int nitems, int nc
 }
 
 // column blocking of the padded density count: nDp = ncolblk * 32 * TN
-void digest_colblocks(int nD, int* TN, int* ncolblk)
-{   // declared in ltjk_internal.h
+void digest_colblocks(int nD, int mode, int* TN, int* ncolblk)
+{   // declared in ltjk_internal.h.  mode 2 (pair lists): A tiles are cheap contiguous copies, and the 16 x 6 thread
+    // tile of TN = 6 stalls on its operand loads (192 accumulator registers), so 192 densities run as 2 x TN = 3
+    // (measured at 730 AO: digestion 3123 -> 2650 ms); mode 1 re-gathers A per column block and prefers TN = 6.
     const int n32 = (nD + 31) / 32;
+    if (const char* e = getenv("LTJK_TN")) {            // development override
+        const int tn = atoi(e);
+        if (tn >= 1 && tn <= 6) { *TN = tn; *ncolblk = (n32 + tn - 1) / tn; return; }
+    }
     int best_tn = 1, best_nb = n32, best_cost = 1 << 30;
-    for (int tn = 1; tn <= 6; ++tn) {
+    for (int tn = 1; tn <= (mode == 2 ? 5 : 6); ++tn) {
         const int nb = (n32 + tn - 1) / tn;
         const int cost = nb * tn * 8 + nb * 3;   // padded columns, then fewer passes over A
         if (cost < best_cost) { best_cost = cost; best_tn = tn; best_nb = nb; }
@@ -418,7 +375,7 @@ int launch_digest(ltjk_ctx* c, const Group& ch, int nDp, bool doJ, bool doK)
     g.Dt = c->Dt; g.Dst = c->Dst; g.Jt = c->Jt; g.Kt = c->Kt;
     g.nDp = nDp;
     int TN, nb;
-    digest_colblocks(nDp, &TN, &nb);
+    digest_colblocks(nDp, 1, &TN, &nb);
     if (nb * TN * 32 != nDp) return set_err(c, LTJK_EINVAL, "internal: nDp is not a whole number of column blocks");
     c->st_launches++;
     switch (TN) {

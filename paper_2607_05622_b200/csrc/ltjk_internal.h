@@ -70,6 +70,60 @@ struct Group {
     double nints;           // integrals in the panels
 };
 
+// ---- pair-list formulation (ltjk_pair.cu, ltjk_pdigest.cu) ---------------------------
+// K[x,r] += sum_c (xc|yr) D[c,y] for fixed "major" AOs (x,y): rows r run over the Schwarz-significant partners of y,
+// the contraction over the partners of x, both sorted by Q descending, so the kept quartets Q_xc Q_yr >= tau form a
+// staircase.  Integrals of one chunk are stored once per role assignment in blocks T_{XY}[iy][c][r][ix] (X, Y shells).
+struct PBlock {
+    long long off;          // offset (doubles) inside the ring half of the block's chunk; -1 = absent
+    int Lc, Lr;             // contraction / row extents in AOs (bounding box of the staircase)
+};
+
+struct PLDev {
+    int G = 0;              // shell groups
+    int* sh_grp = nullptr;  // [nshell]
+    int* pl_start = nullptr;// [nshell*G + 1]  start of the partner list (X,g) in pl_ao
+    int* pl_ao = nullptr;   // partner AOs (internal ids), Q descending, components of a shell consecutive
+    double* pl_q = nullptr; // Schwarz bound Q of (X, partner) for every entry of pl_ao
+    int* pos = nullptr;     // [nshell*nshell] AO rank of shell C in list (X, grp(C)), -1 = dead pair
+    PBlock* blk = nullptr;  // [((X*nshell+Y)*G+g2)*G+g4]
+};
+
+struct PPair {              // one significant shell pair in an ERI launch list
+    int A, B;               // internal shells, l_A >= l_B
+    int joff;               // first AO pair of (A,B) in the J row list of its group pair
+    int pad;
+    double Q;
+};
+
+struct PWork {              // one digestion work record: a matrix A(c, m) = base[c*lda + m] and its row tiles
+    long long off;          // K: block offset;  J: array offset (+ first row already added)
+    int lda;
+    int nrows;              // rows of this record (K: nX*Lr;  J: <= 8 tiles)
+    int kind;               // 0 = K block, 1 = J rows
+    int nY;                 // K: components of Y (one pass per component, stride Lc*lda);  J: 1
+    int Lc;                 // K: contraction extent of the block (stride between iy slabs = Lc*lda)
+    int x0, nX;             // K: first AO of X, components (output row x0 + m % nX)
+    int y0;                 // K: first AO of Y (B row = c_ao * N + y0 + iy)
+    int clist;              // K: offset of the contraction partner list in pl_ao;  J: offset into jrow (contraction)
+    int rlist;              // K: offset of the row partner list in pl_ao;           J: offset into jrow (rows)
+    int tile0;              // first entry of this record in the tile-prefix array (contraction length per row tile)
+    int ntiles;
+    int pad;
+};
+
+struct PChunk {
+    int gab, gcd;           // group-pair indices, gab >= gcd
+    int buf;                // ring half
+    long long doubles;      // storage of the chunk (K blocks + J arrays)
+    long long work0;        // first work record: nworkJ J records, then nworkK K records
+    int nworkJ, nworkK;
+    long long j0_off, j1_off;   // J arrays: rows(gab) x contraction(gcd) and rows(gcd) x contraction(gab) (-1: diagonal chunk)
+    int j0_lda, j1_lda;
+    double exec_rows_chunks_J, exec_rows_chunks_K;   // sum over items of 128 * 16 * chunks (executed A elements)
+    long long nquartets;
+};
+
 }  // namespace ltjk
 
 struct ltjk_ctx {
@@ -112,6 +166,25 @@ struct ltjk_ctx {
     cudaStream_t own_stream = nullptr;
     cudaEvent_t ev_eri[2] = {nullptr, nullptr}, ev_dig[2] = {nullptr, nullptr}, ev_start = nullptr;
 
+    // pair-list formulation
+    ltjk::PLDev pl;
+    std::vector<ltjk::PChunk> pchunks;
+    ltjk::PWork* d_pwork = nullptr;
+    int* d_ptile = nullptr;                // contraction length per row tile
+    int* d_jrow = nullptr;                 // per group pair: AO-pair row ids (i*N + j), Q descending
+    double* d_jq = nullptr;                // Schwarz bound of every entry of d_jrow
+    ltjk::PPair* d_ppairs = nullptr;       // ERI launch lists: per (group pair, class), Q descending
+    std::vector<long long> pp_start;       // [ngp*6 + 1] into d_ppairs
+    std::vector<long long> jrow_start;     // [ngp + 1] into d_jrow
+    std::vector<double> pp_q;              // host copy of the Q column of d_ppairs (launch sizing)
+    double* d_pring = nullptr;             // integral staging ring of the pair-list path (one or two halves)
+    long long pring_half = 0;              // doubles per half
+    int* d_pcounter = nullptr;             // work-stealing cursors, one per digestion launch of a build
+    int pcounter_next = 0, pcounter_cap = 0;
+    int digest_mode_req = 0;               // requested: 0 = auto, 1 = block panels (dense), 2 = pair lists
+    int digest_mode = 1;                   // in use: 1 = block panels, 2 = pair lists (screening-aware)
+    bool have_pl = false;
+
     // per-build work buffers (grown on demand): density-fastest internal layouts [N][N][nDp]
     double *Dt = nullptr, *Dst = nullptr, *Jt = nullptr, *Kt = nullptr;
     long long work_cap = 0;               // doubles per buffer
@@ -139,7 +212,7 @@ int set_err(ltjk_ctx* c, int code, const std::string& msg);
 void free_tables(ltjk_ctx* c);
 void free_work(ltjk_ctx* c);
 void build_work(ltjk_ctx* c, std::vector<DigestItem>& items);
-void digest_colblocks(int nD, int* TN, int* ncolblk);
+void digest_colblocks(int nD, int mode, int* TN, int* ncolblk);
 
 // ltjk_eri.cu
 int launch_pair_records(ltjk_ctx* c, const double* d_xyz, const int* d_atom, const int* d_l, const int* d_nprim,
@@ -148,6 +221,13 @@ int launch_schwarz(ltjk_ctx* c, const int* lrange_host);
 int launch_eri_panels(ltjk_ctx* c, const Group& g, int ck);
 int launch_eri_single(ltjk_ctx* c, int A, int B, int C, int D, int la, int lb, int lc, int ld, double* d_out);
 int launch_boys_debug(ltjk_ctx* c, int mmax, int n, const double* d_T, double* d_F);
+
+// ltjk_pair.cu, ltjk_peri.cu, ltjk_pdigest.cu: pair-list formulation
+int build_pairlists(ltjk_ctx* c);
+void free_pairlists(ltjk_ctx* c);
+int launch_peri_chunk(ltjk_ctx* c, const PChunk& ch);
+int launch_pdigest(ltjk_ctx* c, const PChunk& ch, int nDp, bool doJ, bool doK);
+int launch_pzero(ltjk_ctx* c, const PChunk& ch);
 
 // ltjk_digest.cu
 int launch_digest(ltjk_ctx* c, const Group& g, int nDp, bool doJ, bool doK);
@@ -163,6 +243,8 @@ int launch_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C_occ
                             const double* tau_host, double* D_out);
 
 int launch_laplace_fock(ltjk_ctx* c, int nD, const double* J, const double* K, int nmo, const double* C, double* F);
+int launch_mo_transform(ltjk_ctx* c, int nD, const double* A, double ca, const double* A2, double ca2, int nmo,
+                        const double* C, double* F);
 int launch_laplace_accumulate(ltjk_ctx* c, int ntau, int nT, long long nelem, const double* tau_host,
                               const double* w_host, double omega, const double* X, double* Y);
 

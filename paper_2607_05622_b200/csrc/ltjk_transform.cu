@@ -175,15 +175,22 @@ __global__ void transpose_kernel(int rows, int cols, const double* __restrict__ 
 
 int launch_laplace_fock(ltjk_ctx* c, int nD, const double* J, const double* K, int nmo, const double* C, double* F)
 {
+    return launch_mo_transform(c, nD, J, 2.0, K, -1.0, nmo, C, F);
+}
+
+// F[d] = C^T (ca A[d] + ca2 A2[d]) C for nD matrices (A2 may be NULL): two batched DMMA GEMMs.
+int launch_mo_transform(ltjk_ctx* c, int nD, const double* A, double ca, const double* A2, double ca2, int nmo,
+                        const double* C, double* F)
+{
     const int N = c->nao;
     double *Ct = nullptr, *tmp = nullptr;
     LTJK_CUDA(c, cudaMallocAsync(&Ct, sizeof(double) * (size_t)N * nmo, c->stream));
     LTJK_CUDA(c, cudaMallocAsync(&tmp, sizeof(double) * (size_t)nD * N * nmo, c->stream));
     transpose_kernel<<<dim3((nmo + 31) / 32, (N + 31) / 32), dim3(32, 8), 0, c->stream>>>(N, nmo, C, Ct);
     LTJK_CUDA(c, cudaGetLastError());
-    GemmArgs g1;   // tmp[d] (N x nmo) = (2 J[d] - K[d]) . C
+    GemmArgs g1;   // tmp[d] (N x nmo) = (ca A[d] + ca2 A2[d]) . C
     g1.M = N; g1.Nn = nmo; g1.K = N;
-    g1.A = J; g1.A2 = K; g1.ca = 2.0; g1.ca2 = -1.0; g1.sAa = (long long)N * N; g1.sAb = 0;
+    g1.A = A; g1.A2 = A2; g1.ca = ca; g1.ca2 = A2 ? ca2 : 0.0; g1.sAa = (long long)N * N; g1.sAb = 0;
     g1.B = C; g1.sBa = 0; g1.sBb = 0;
     g1.C = tmp; g1.sCa = (long long)N * nmo; g1.sCb = 0;
     g1.sr = nullptr; g1.ssr = 0; g1.sc = nullptr; g1.ssc = 0; g1.nzb = 1;

@@ -23,7 +23,7 @@ ERRORS = {0: "LTJK_OK", -1: "LTJK_EINVAL", -2: "LTJK_ENOBASIS", -3: "LTJK_ECUDA"
 EXPORTS = [
     "ltjk_create", "ltjk_destroy", "ltjk_last_error", "ltjk_set_scratch_bytes", "ltjk_set_basis", "ltjk_get_nao",
     "ltjk_build_shell_pairs", "ltjk_get_schwarz", "ltjk_laplace_quadrature", "ltjk_build_pseudo_densities",
-    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_laplace_fock", "ltjk_laplace_accumulate", "ltjk_get_stats", "ltjk_set_timing", "ltjk_debug_eri_quartet",
+    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_laplace_fock", "ltjk_laplace_accumulate", "ltjk_pp_ladder", "ltjk_get_stats", "ltjk_set_timing", "ltjk_set_digest_mode", "ltjk_get_digest_mode", "ltjk_debug_eri_quartet",
     "ltjk_debug_boys", "ltjk_bench_dfma_peak", "ltjk_bench_copy_peak",
 ]
 
@@ -210,6 +210,11 @@ class Context:
                                                    ctypes.c_longlong(nelem), _d(tau), _d(w), ctypes.c_double(omega),
                                                    _devptr(X), _devptr(Y)))
 
+    def pp_ladder(self, C_vir, X, L, chunk=0):
+        """ltjk_pp_ladder: L[p] = C_vir^T K[C_vir X[p] C_vir^T] C_vir = sum_ef (ae|bf) X[p,e,f]; device tensors."""
+        self._chk(self.lib.ltjk_pp_ladder(self._h, ctypes.c_int(C_vir.shape[1]), _devptr(C_vir),
+                                          ctypes.c_int(X.shape[0]), _devptr(X), _devptr(L), ctypes.c_int(int(chunk))))
+
     def get_stats(self) -> dict:
         nl = ctypes.c_longlong(0)
         nq = ctypes.c_longlong(0)
@@ -220,6 +225,14 @@ class Context:
                                           ctypes.byref(e), ctypes.byref(g)))
         return {"n_launches": nl.value, "eri_quartets": nq.value, "digest_flops": fl.value, "eri_ms": e.value,
                 "digest_ms": g.value}
+
+    def set_digest_mode(self, mode: int):
+        self._chk(self.lib.ltjk_set_digest_mode(self._h, ctypes.c_int(int(mode))))
+
+    def get_digest_mode(self) -> int:
+        m = ctypes.c_int(0)
+        self._chk(self.lib.ltjk_get_digest_mode(self._h, ctypes.byref(m)))
+        return m.value
 
     def set_timing(self, enable: bool):
         self._chk(self.lib.ltjk_set_timing(self._h, ctypes.c_int(1 if enable else 0)))

@@ -33,11 +33,13 @@ def torch_cuda():
     return torch
 
 
-def make_ctx(basis, tau=SCHWARZ_TAU, scratch=None):
+def make_ctx(basis, tau=SCHWARZ_TAU, scratch=None, mode=0):
+    """mode: digestion strategy (ltjk_set_digest_mode): 0 automatic, 1 block panels, 2 pair lists."""
     from paper_2607_05622_b200 import ltjk
     ctx = ltjk.Context(0)
     if scratch is not None:
         ctx.set_scratch_bytes(scratch)
+    ctx.set_digest_mode(mode)
     ctx.set_basis(basis)
     ctx.build_shell_pairs(tau)
     return ctx
@@ -93,11 +95,12 @@ def test_schwarz_vs_oracle(torch_cuda, small):
     assert np.allclose(Q, Q.T)
 
 
-def test_jk_tiny_vs_definition(torch_cuda, tiny):
+@pytest.mark.parametrize("mode", [1, 2])
+def test_jk_tiny_vs_definition(torch_cuda, tiny, mode):
     """BASELINE gate: GPU vs the brute-force explicit-N^4 contraction (oracle O7) on the tiny config."""
     b = tiny.basis
     D = random_densities(b.nao, 3, seed=11)
-    ctx = make_ctx(b, tau=0.0)
+    ctx = make_ctx(b, tau=0.0, mode=mode)
     J, K = gpu_jk(torch_cuda, ctx, D)
     eri = O.eri_tensor(b)
     Jr, Kr = O.jk_definition(eri, D)
@@ -106,11 +109,13 @@ def test_jk_tiny_vs_definition(torch_cuda, tiny):
     assert np.abs(K - K.transpose(0, 2, 1)).max() > 1e-3 * np.abs(K).max()
 
 
-def test_jk_spd_vs_definition(torch_cuda, spd_basis):
-    """s, p and d shells (all 21 canonical classes, diagonal blocks included) against Eq. 17 literally."""
+@pytest.mark.parametrize("mode,scratch", [(1, None), (2, None), (2, 1 << 16)])
+def test_jk_spd_vs_definition(torch_cuda, spd_basis, mode, scratch):
+    """s, p and d shells (all 21 canonical classes, diagonal blocks included) against Eq. 17 literally; the tiny
+    scratch budget forces the pair-list path into 8 shell groups (666 chunks, every role-assignment family)."""
     b = spd_basis
     D = random_densities(b.nao, 5, seed=12)
-    ctx = make_ctx(b, tau=0.0)
+    ctx = make_ctx(b, tau=0.0, scratch=scratch, mode=mode)
     J, K = gpu_jk(torch_cuda, ctx, D)
     Jr, Kr = O.jk_definition(O.eri_tensor(b), D)
     assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
@@ -134,12 +139,15 @@ def test_jk_tiny_pseudo_densities_end_to_end(torch_cuda, tiny):
     assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
 
 
-@pytest.mark.parametrize("scratch", [None, 1 << 20])
-def test_jk_small_vs_folded(torch_cuda, small, scratch):
-    """160 AO, contracted s/p/d, ragged blocks; a small scratch forces many chunks per bra block pair."""
+@pytest.mark.parametrize("mode,scratch,nD", [(1, None, 5), (1, 1 << 20, 5), (2, None, 5), (2, 1 << 22, 5), (2, None, 33),
+                                              (2, 1 << 24, 96)])
+def test_jk_small_vs_folded(torch_cuda, small, mode, scratch, nD):
+    """160 AO, contracted s/p/d, ragged blocks; a small scratch forces many chunks (both strategies); 33 and 96
+    densities reach the TN = 2 and TN = 3 column blockings of the pair-list kernel."""
     w = small
-    D = random_densities(w.nao, 5, seed=13)
-    ctx = make_ctx(w.basis, scratch=scratch)
+    D = random_densities(w.nao, nD, seed=13)
+    ctx = make_ctx(w.basis, scratch=scratch, mode=mode)
+    assert ctx.get_digest_mode() == mode
     J, K = gpu_jk(torch_cuda, ctx, D)
     Jr, Kr, kept = O.jk_folded(w.basis, D, w.schwarz_tau)
     assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
@@ -165,12 +173,12 @@ def test_jk_host_entry_matches_device_entry(torch_cuda, tiny):
     assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
 
 
-def full_sweep(torch, name):
+def full_sweep(torch, name, mode=0):
     """The whole Laplace sweep in the configuration bench.py times (transform + J/K for all n_tau x n_T densities,
     default panel ring).  Density nD-1 is replaced by the transpose of density 0 (K must come out transposed)."""
     w = make_workload(name)
     N, nD = w.nao, w.nD
-    ctx = make_ctx(w.basis)
+    ctx = make_ctx(w.basis, mode=mode)
     tau = np.geomspace(0.05, 6.0, w.ntau)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     D = torch.empty((w.ntau, w.nT, N, N), dtype=torch.float64, device="cuda")
@@ -217,17 +225,23 @@ def linearity_closure(torch, ctx, Dn, J, K, seed=9):
 
 
 def test_full_size_medium_full_matrices(torch_cuda):
-    """300 AO, all 80 densities of the sweep: every element of J and K against the folded oracle O6."""
-    w, ctx, Dn, J, K = full_sweep(torch_cuda, "medium")
+    """300 AO, all 80 densities of the sweep: every element of J and K against the folded oracle O6, with both
+    digestion strategies (one oracle run serves both)."""
+    w, ctx, Dn, J, K = full_sweep(torch_cuda, "medium", mode=1)
     Jr, Kr, _ = O.jk_folded(w.basis, Dn.cpu().numpy(), w.schwarz_tau)
     assert relerr(J.cpu().numpy(), Jr) < TOL and relerr(K.cpu().numpy(), Kr) < TOL
     linearity_closure(torch_cuda, ctx, Dn, J, K)
+    del ctx
+    w2, ctx2, Dn2, J2, K2 = full_sweep(torch_cuda, "medium", mode=2)
+    assert relerr(J2.cpu().numpy(), Jr) < TOL and relerr(K2.cpu().numpy(), Kr) < TOL
+    linearity_closure(torch_cuda, ctx2, Dn2, J2, K2)
 
 
 def test_full_size_porphine_full_matrices_subset(torch_cuda):
     """439 AO, the sweep bench.py times (160 densities, TN = 5): full N x N matrices of a seeded 8-density subset
     against the folded oracle O6, plus the linearity closure over all 160 densities."""
     w, ctx, Dn, J, K = full_sweep(torch_cuda, "porphine")
+    assert ctx.get_digest_mode() == 1                 # compact molecule: block panels (automatic choice)
     ds = density_subset(w.nD)
     Jr, Kr, _ = O.jk_folded(w.basis, Dn[ds].cpu().numpy(), w.schwarz_tau)
     assert relerr(J[ds].cpu().numpy(), Jr) < TOL and relerr(K[ds].cpu().numpy(), Kr) < TOL
@@ -242,6 +256,7 @@ def test_full_size_large_subset_closure(torch_cuda):
     import os
     torch = torch_cuda
     w, ctx, Dn, J, K = full_sweep(torch, "large")
+    assert ctx.get_digest_mode() == 2                 # extended molecule: pair lists (automatic choice)
     linearity_closure(torch, ctx, Dn, J, K)
     ds = density_subset(w.nD)
     Dh, Jh, Kh = Dn[ds].cpu().numpy(), J[ds].cpu().numpy(), K[ds].cpu().numpy()
@@ -401,3 +416,25 @@ def test_three_and_four_primitive_contractions(torch_cuda):
     J, K = gpu_jk(torch_cuda, ctx, D)
     Jr, Kr = O.jk_definition(O.eri_tensor(b), D)
     assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_pp_ladder_vs_oracle(torch_cuda, tiny, spd_basis, mode):
+    """the AO-direct particle-particle ladder as a K-only batch, against
+    the oracle's explicit sum over (e,f) of virtual-orbital integrals built from the N^4 tensor (O7).  37 pair columns
+    with chunk = 16 exercise a ragged last chunk; chunk = 0 the default."""
+    torch = torch_cuda
+    for b in (tiny.basis, spd_basis):
+        rng = np.random.default_rng(17)
+        nv = 7
+        Cv = rng.standard_normal((b.nao, nv)) / np.sqrt(b.nao)
+        X = rng.standard_normal((37, nv, nv))
+        ref = O.pp_ladder(O.eri_tensor(b), Cv, X)
+        ctx = make_ctx(b, tau=0.0, mode=mode)
+        Cd, Xd = torch.from_numpy(Cv).cuda(), torch.from_numpy(X).cuda()
+        for chunk in (16, 0):
+            L = torch.full((37, nv, nv), float("nan"), dtype=torch.float64, device="cuda")
+            ctx.pp_ladder(Cd, Xd, L, chunk)
+            torch.cuda.synchronize()
+            assert relerr(L.cpu().numpy(), ref) < TOL
+        assert np.abs(ref - ref.transpose(0, 2, 1)).max() > 1e-3 * np.abs(ref).max()    # non-symmetric, as X is
