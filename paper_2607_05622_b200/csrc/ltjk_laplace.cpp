@@ -6,7 +6,7 @@
 // (tau = tau^/xmin, w = w^/xmin).  Method (this library's own code; the CPU oracle is an independent Python/mpmath
 // implementation in 80-digit arithmetic, reading A8):
 //   1. start on a wide interval [1,R0]: Levenberg-Marquardt least squares in (log tau, log w) on a logarithmic
-//      grid, from the trapezoid rule for 1/x = int exp(-x e^s) e^s ds; accepted only if its error curve has
+//      grid (80-bit long double: only a start guess, 2x faster than quad), from the trapezoid rule for 1/x = int exp(-x e^s) e^s ds; accepted only if its error curve has
 //      2k+1 alternating extrema (else another R0 is tried);
 //   2. Remez exchange: Newton on E(x_j) = (-1)^j delta for (tau, w, delta), then every interior x_j moves to the
 //      neighbouring extremum of E; repeated to convergence;
@@ -43,84 +43,92 @@ real derr_at(const Grid& g, real x)
     return -1 / (x * x) + s;
 }
 
+template <class R> inline R absr(R x) { return x < 0 ? -x : x; }
 // Gaussian elimination with partial pivoting; A is n x n row-major, b overwritten with the solution.
-bool solve(std::vector<real>& A, vec& b, int n)
+template <class R>
+bool solve_t(std::vector<R>& A, std::vector<R>& b, int n)
 {
     for (int c = 0; c < n; ++c) {
         int p = c;
-        for (int r = c + 1; r < n; ++r) if (qabs(A[r * n + c]) > qabs(A[p * n + c])) p = r;
+        for (int r = c + 1; r < n; ++r) if (absr(A[r * n + c]) > absr(A[p * n + c])) p = r;
         if (A[p * n + c] == 0) return false;
         if (p != c) { for (int j = 0; j < n; ++j) std::swap(A[c * n + j], A[p * n + j]); std::swap(b[c], b[p]); }
         for (int r = c + 1; r < n; ++r) {
-            const real f = A[r * n + c] / A[c * n + c];
+            const R f = A[r * n + c] / A[c * n + c];
             if (f == 0) continue;
             for (int j = c; j < n; ++j) A[r * n + j] -= f * A[c * n + j];
             b[r] -= f * b[c];
         }
     }
     for (int r = n - 1; r >= 0; --r) {
-        real s = b[r];
+        R s = b[r];
         for (int j = r + 1; j < n; ++j) s -= A[r * n + j] * b[j];
         b[r] = s / A[r * n + r];
     }
     return true;
 }
 
+
+bool solve(std::vector<real>& A, vec& b, int n) { return solve_t<real>(A, b, n); }
+
 // Step 1: LM least squares on a log grid of [1,R0] in p = (log tau, log w).
-bool ls_start(int k, real R0, Grid& g)
+bool ls_start(int k, real R0q, Grid& g)
 {
+    typedef long double lreal;
+    typedef std::vector<lreal> lvec;
+    const lreal R0 = (lreal)R0q;
     const int n = 400, np = 2 * k;
-    vec xg(n);
-    for (int i = 0; i < n; ++i) xg[i] = qexp(qlog(R0) * i / (n - 1));
-    const real lo = 2.5Q, hi = 3.0Q, hh = (qlog(R0) + lo + hi) / k;
-    vec p(np);
-    for (int a = 0; a < k; ++a) { p[a] = -qlog(R0) - lo + hh * (a + 0.5Q); p[k + a] = qlog(hh) + p[a]; }
-    auto residual = [&](const vec& q, vec& r) {
-        real s2 = 0;
+    lvec xg(n);
+    for (int i = 0; i < n; ++i) xg[i] = expl(logl(R0) * i / (n - 1));
+    const lreal lo = 2.5L, hi = 3.0L, hh = (logl(R0) + lo + hi) / k;
+    lvec p(np);
+    for (int a = 0; a < k; ++a) { p[a] = -logl(R0) - lo + hh * (a + 0.5L); p[k + a] = logl(hh) + p[a]; }
+    auto residual = [&](const lvec& q, lvec& r) {
+        lreal s2 = 0;
         for (int i = 0; i < n; ++i) {
-            real s = 0;
-            for (int a = 0; a < k; ++a) s += qexp(q[k + a] - xg[i] * qexp(q[a]));
+            lreal s = 0;
+            for (int a = 0; a < k; ++a) s += expl(q[k + a] - xg[i] * expl(q[a]));
             r[i] = 1 / xg[i] - s;
             s2 += r[i] * r[i];
         }
         return s2;
     };
-    vec r(n), rn(n), pn(np);
-    real f = residual(p, r), lam = 1e-3Q;
-    std::vector<real> Jm((size_t)n * np), A((size_t)np * np);
-    vec gvec(np), d(np);
+    lvec r(n), rn(n), pn(np);
+    lreal f = residual(p, r), lam = 1e-3L;
+    std::vector<lreal> Jm((size_t)n * np), A((size_t)np * np);
+    lvec gvec(np), d(np);
     for (int it = 0; it < 3000; ++it) {
         for (int i = 0; i < n; ++i)
             for (int a = 0; a < k; ++a) {
-                const real t = qexp(p[a]), e = qexp(p[k + a] - xg[i] * t);
+                const lreal t = expl(p[a]), e = expl(p[k + a] - xg[i] * t);
                 Jm[(size_t)i * np + a] = e * xg[i] * t;      // d r_i / d log tau_a
                 Jm[(size_t)i * np + k + a] = -e;              // d r_i / d log w_a
             }
         for (int a = 0; a < np; ++a) {
-            real s = 0;
+            lreal s = 0;
             for (int i = 0; i < n; ++i) s += Jm[(size_t)i * np + a] * r[i];
             gvec[a] = s;
             for (int b = a; b < np; ++b) {
-                real t = 0;
+                lreal t = 0;
                 for (int i = 0; i < n; ++i) t += Jm[(size_t)i * np + a] * Jm[(size_t)i * np + b];
                 A[(size_t)a * np + b] = A[(size_t)b * np + a] = t;
             }
         }
         bool improved = false;
         for (int tries = 0; tries < 40; ++tries) {
-            std::vector<real> M = A;
+            std::vector<lreal> M = A;
             for (int a = 0; a < np; ++a) { M[(size_t)a * np + a] += lam * A[(size_t)a * np + a]; d[a] = -gvec[a]; }
-            if (solve(M, d, np)) {
-                real big = 0;
-                for (int a = 0; a < np; ++a) big = std::max<real>(big, qabs(d[a]));
-                const real sc = big > 2 ? 2 / big : 1;
+            if (solve_t<lreal>(M, d, np)) {
+                lreal big = 0;
+                for (int a = 0; a < np; ++a) big = std::max<lreal>(big, fabsl(d[a]));
+                const lreal sc = big > 2 ? 2 / big : 1;
                 for (int a = 0; a < np; ++a) pn[a] = p[a] + sc * d[a];
-                const real fn = residual(pn, rn);
+                const lreal fn = residual(pn, rn);
                 if (fn < f) {
-                    const real rel = (f - fn) / f;
-                    p = pn; r = rn; f = fn; lam = std::max<real>(lam / 3, 1e-30Q);
+                    const lreal rel = (f - fn) / f;
+                    p = pn; r = rn; f = fn; lam = std::max<lreal>(lam / 3, 1e-30L);
                     improved = true;
-                    if (rel < 1e-14Q) it = 1 << 30;
+                    if (rel < 1e-14L) it = 1 << 30;
                     break;
                 }
             }
@@ -132,7 +140,7 @@ bool ls_start(int k, real R0, Grid& g)
     std::vector<std::pair<double, int>> order(k);
     for (int a = 0; a < k; ++a) order[a] = {(double)p[a], a};
     std::sort(order.begin(), order.end());
-    for (int a = 0; a < k; ++a) { g.tau[a] = qexp(p[order[a].second]); g.w[a] = qexp(p[k + order[a].second]); }
+    for (int a = 0; a < k; ++a) { g.tau[a] = (real)expl(p[order[a].second]); g.w[a] = (real)expl(p[k + order[a].second]); }
     return true;
 }
 
@@ -258,7 +266,7 @@ bool minimax(int k, real R, Grid& g, real& delta)
 
 extern "C" int ltjk_laplace_quadrature(double xmin, double xmax, int npts, double* t, double* w, double* maxerr)
 {
-    if (!(xmin > 0.0) || !(xmax > xmin) || npts < 1 || npts > 16 || !t || !w) return LTJK_EINVAL;
+    if (!(xmin > 0.0) || !(xmax > xmin) || npts < 2 || npts > 14 || !t || !w) return LTJK_EINVAL;
     Grid g;
     real delta = 0;
     const real R = (real)xmax / (real)xmin;
