@@ -249,10 +249,10 @@ def test_full_size_porphine_full_matrices_subset(torch_cuda):
 
 
 def test_full_size_large_subset_closure(torch_cuda):
-    """730 AO, 192 densities (TN = 6): SURVEY 8(d)'s stated fallback, reported as "subset+closure": the GPU linearity
-    closure over all 192 densities, plus the oracle on an 8-density subset.  In the default tier the oracle evaluates
-    Eq. 17 on 120 sampled shell-pair blocks (stratified over the nine l-pair classes); with LTJK_SLOW=1 it is the
-    full-matrix folded oracle O6 on the same subset (13-15 min on 16 cores; run once per round, log in profiles/)."""
+    """730 AO, 192 densities, pair-list digestion: SURVEY 8(d)'s stated fallback, reported as "subset+closure": the GPU
+    linearity closure over all 192 densities, plus the full N x N matrices of a seeded 8-density subset against the
+    folded oracle O6 (about 6.5 min on the 16 host cores of the GPU box).  LTJK_FAST=1 replaces the full-matrix oracle
+    by Eq. 17 on 120 sampled shell-pair blocks (stratified over the nine l-pair classes, about 1.5 min)."""
     import os
     torch = torch_cuda
     w, ctx, Dn, J, K = full_sweep(torch, "large")
@@ -261,7 +261,7 @@ def test_full_size_large_subset_closure(torch_cuda):
     ds = density_subset(w.nD)
     Dh, Jh, Kh = Dn[ds].cpu().numpy(), J[ds].cpu().numpy(), K[ds].cpu().numpy()
     b = w.basis
-    if os.environ.get("LTJK_SLOW") == "1":
+    if os.environ.get("LTJK_FAST") != "1":
         Jr, Kr, _ = O.jk_folded(b, Dh, w.schwarz_tau)
         ej, ek = relerr(Jh, Jr), relerr(Kh, Kr)
         print("large full-matrix subset: relerr J %.3e K %.3e over densities %s" % (ej, ek, ds))
@@ -438,3 +438,41 @@ def test_pp_ladder_vs_oracle(torch_cuda, tiny, spd_basis, mode):
             torch.cuda.synchronize()
             assert relerr(L.cpu().numpy(), ref) < TOL
         assert np.abs(ref - ref.transpose(0, 2, 1)).max() > 1e-3 * np.abs(ref).max()    # non-symmetric, as X is
+
+
+def test_level2_density_from_laplace_fock(torch_cuda, tiny):
+    """SURVEY 8(f) N1, last link (Eq. 15 with R^(2); Alg. 1): the occupied-virtual block of the
+    Laplace-Fock matrix F~^alpha = C^T (2 J - K) C of level 1 is fed back as the amplitude R^(2) of the level-2
+    pseudo-density at the same grid point.  Whole chain on the GPU against the whole chain in the oracle."""
+    torch = torch_cuda
+    w = tiny
+    N, no = w.nao, w.nocc
+    tau = np.linspace(0.2, 2.5, 3)
+    T = np.concatenate([w.T, 0.5 * w.T[::-1] + 0.01], axis=0)[:2]            # two amplitude sets
+    nT = T.shape[0]
+    ctx = make_ctx(w.basis)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Co, Cv, eo, ev = dev(w.C_occ), dev(w.C_vir), dev(w.eps_occ), dev(w.eps_vir)
+    C = np.ascontiguousarray(np.concatenate([w.C_occ, w.C_vir], axis=1))
+    D1 = torch.empty((len(tau), nT, N, N), dtype=torch.float64, device="cuda")
+    ctx.build_pseudo_densities(Co, Cv, eo, ev, dev(T), tau, D1)
+    D1n = D1.view(-1, N, N)
+    J = torch.empty_like(D1n)
+    K = torch.empty_like(D1n)
+    ctx.jk_build(D1n, J, K)
+    F = torch.empty((len(tau) * nT, N, N), dtype=torch.float64, device="cuda")
+    ctx.laplace_fock(J, K, dev(C), F)
+    D2 = torch.empty((len(tau), nT, N, N), dtype=torch.float64, device="cuda")
+    for a in range(len(tau)):
+        R2 = F[a * nT:(a + 1) * nT, :no, no:].contiguous()                  # ov block of F~^alpha
+        ctx.build_pseudo_densities(Co, Cv, eo, ev, R2, tau[a:a + 1], D2[a:a + 1])
+    torch.cuda.synchronize()
+    # oracle chain
+    D1r = O.pseudo_densities_loops(w.C_occ, w.C_vir, w.eps_occ, w.eps_vir, T, tau).reshape(-1, N, N)
+    Jr, Kr, _ = O.jk_folded(w.basis, D1r, w.schwarz_tau)
+    Fr = O.laplace_fock(Jr, Kr, C)
+    D2r = np.stack([O.pseudo_densities_loops(w.C_occ, w.C_vir, w.eps_occ, w.eps_vir,
+                                             Fr[a * nT:(a + 1) * nT, :no, no:], tau[a:a + 1])[0] for a in range(len(tau))])
+    assert relerr(F.cpu().numpy(), Fr) < TOL
+    assert relerr(D2.cpu().numpy().reshape(-1, N, N), D2r.reshape(-1, N, N)) < TOL
+    assert np.abs(D2r).max() > 0
