@@ -385,10 +385,47 @@ def main():
               "eri_fp64_flops_per_sweep_ncu": committed_ncu("eri_fp64_flops_per_sweep_%s" % w.name),
               "gpu": torch.cuda.get_device_name(local), "hbm_copy_gbs_measured": hbm_gbs,
               "dfma_peak_tflops_measured": peak_tf}
-    # free the headline workload before the 730-AO sub-run
+    # free the headline workload before the sub-runs
     del rep, Dn, D1, J1, K1
     ctx.close()
     torch.cuda.empty_cache()
+    if world == 1 and w.name != "large":
+        # callers that cannot batch: one Laplace point per call with the geometry-frozen integral cache
+        # (ltjk_set_resident), and the N3 particle-particle ladder (K-only batches of 160 pair columns)
+        c2 = ltjk.Context(local, stream)
+        c2.set_resident(True)
+        c2.set_basis(w.basis)
+        c2.build_shell_pairs(w.schwarz_tau)
+        rng = np.random.default_rng(7)
+        D1 = torch.from_numpy(1e-2 * rng.standard_normal((w.nT, N, N))).cuda()
+        J1 = torch.empty_like(D1)
+        K1 = torch.empty_like(D1)
+        c2.jk_build(D1, J1, K1)                      # first build fills the cache
+        torch.cuda.synchronize()
+        e0.record(stream)
+        c2.jk_build(D1, J1, K1)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        config["one_laplace_point_per_call_resident"] = {
+            "n_D": int(w.nT), "ms": e0.elapsed_time(e1), "builds_per_s": w.nT / (e0.elapsed_time(e1) * 1e-3),
+            "note": "integral panels of the geometry kept in HBM (opt-in cache, not the headline path)"}
+        npair = 320
+        Cv = torch.from_numpy(np.ascontiguousarray(w.C_vir)).cuda()
+        X = torch.from_numpy(1e-2 * rng.standard_normal((npair, w.nvir, w.nvir))).cuda()
+        Lo = torch.empty_like(X)
+        c2.pp_ladder(Cv, X, Lo)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        c2.pp_ladder(Cv, X, Lo)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        config["pp_ladder"] = {"pair_columns": npair, "nvir": int(w.nvir), "ms": e0.elapsed_time(e1),
+                               "pair_columns_per_s": npair / (e0.elapsed_time(e1) * 1e-3),
+                               "note": "L[p,a,b] = sum_ef (ae|bf) X[p,e,f] as K-only builds (SURVEY 8(f) N3), resident panels"}
+        launches += 2 * (c2.get_stats()["n_launches"])
+        del D1, J1, K1, X, Lo
+        c2.close()
+        torch.cuda.empty_cache()
     if world == 1 and not args.no_large and w.name != "large":
         wl = make_workload("large")
         s2 = ClockSampler(local)

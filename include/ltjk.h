@@ -152,6 +152,12 @@ int ltjk_set_timing(ltjk_ctx* ctx, int enable);
  *      mode 1 otherwise.
  * Results are the same sums up to rounding order.  Returns LTJK_EINVAL for other values. */
 int ltjk_set_digest_mode(ltjk_ctx* ctx, int mode);
+/* Geometry-frozen integral cache ("geometry-frozen caches for per-step reuse"), read by the NEXT
+ * ltjk_build_shell_pairs; strategy 1 only.  enable != 0: if all canonical integral panels of the geometry fit in
+ * 60 % of the free device memory (439 AO: 41 GB) they are generated by the first ltjk_jk_build and kept; later builds
+ * on the same geometry only digest.  Meant for callers that cannot batch their densities (one Laplace point per
+ * call, pp-ladder chunks).  Off by default: the path is integral-direct.  Silently stays off if it does not fit. */
+int ltjk_set_resident(ltjk_ctx* ctx, int enable);
 /* The strategy (1 or 2) chosen by the last ltjk_build_shell_pairs; LTJK_ENOBASIS before it. */
 int ltjk_get_digest_mode(const ltjk_ctx* ctx, int* mode);
 

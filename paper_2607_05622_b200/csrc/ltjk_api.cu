@@ -104,7 +104,7 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
         items.insert(items.end(), jitems.begin(), jitems.end());
         items.insert(items.end(), kitems.begin(), kitems.end());
         jitems.clear(); kitems.clear();
-        g.buf = (int)(c->groups.size() & 1);
+        g.buf = c->resident ? 0 : (int)(c->groups.size() & 1);
         c->groups.push_back(g);
         open = false;
     };
@@ -121,7 +121,7 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
                 g = Group();
                 g.sub0 = (int)c->subs.size(); g.nsub = 0; g.cb = cb; g.nquartets = 0; g.nints = 0.0;
                 for (int k = 0; k < 6; ++k) g.maxkets[k] = 0;
-                used = 0;
+                if (!c->resident) used = 0;             // resident: every group keeps its own region of the panel store
                 open = true;
             }
             int r1 = r0 + 1;

@@ -153,6 +153,17 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     long long total = c->koff[npair] * c->koff[npair];      // never need more than everything at once
     c->panel_half = std::max<long long>(std::min<long long>(bytes / 16, total), maxpanel);
     c->panel_cap = 2 * c->panel_half;
+    // resident panels (ltjk_set_resident): one region per group, all canonical panels = sum_r nIJ(r) * koff[r+1] doubles
+    c->resident = false; c->panels_valid = false;
+    if (c->resident_req && panels) {
+        long long all = 0;
+        for (int r = 0; r < npair; ++r) all += (c->koff[r + 1] - c->koff[r]) * c->koff[r + 1];
+        if ((double)all * sizeof(double) <= 0.6 * (double)freeb) {
+            c->resident = true;
+            c->panel_half = std::max<long long>(all, maxpanel);
+            c->panel_cap = c->panel_half;
+        }
+    }
     std::vector<DigestItem> items;
     if (panels) {
         LTJK_CUDA(c, cudaMalloc(&c->d_panel, sizeof(double) * c->panel_cap));
@@ -275,8 +286,9 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
     for (const Group& gr : c->groups) {
         if (!c->timing && gi >= 2) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[gr.buf], 0));
         if (c->timing) cudaEventRecord(e0, c->stream);
-        for (int ck = 0; ck <= gr.cb; ++ck)
-            if ((rc = launch_eri_panels(c, gr, ck))) return rc;
+        if (!(c->resident && c->panels_valid))
+            for (int ck = 0; ck <= gr.cb; ++ck)
+                if ((rc = launch_eri_panels(c, gr, ck))) return rc;
         if (c->timing) cudaEventRecord(e1, c->stream);
         else {
             LTJK_CUDA(c, cudaEventRecord(c->ev_eri[gr.buf], c->eri_stream));
@@ -296,6 +308,7 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
         c->st_digest_flops += 2.0 * gr.nints * nDp * ((J ? 2.0 : 0.0) + (K ? 8.0 : 0.0));   // images applied (folded ones included)
     }
     if (c->timing) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2); }
+    if (c->resident) c->panels_valid = true;            // the panels of this geometry stay in HBM for the next build
     if ((rc = launch_unpack_results(c, nD, nDp, J, K))) return rc;
     return LTJK_OK;
 }
@@ -448,6 +461,13 @@ int ltjk_set_digest_mode(ltjk_ctx* c, int mode)
 {
     if (!c || mode < 0 || mode > 2) return LTJK_EINVAL;
     c->digest_mode_req = mode;
+    return LTJK_OK;
+}
+
+int ltjk_set_resident(ltjk_ctx* c, int enable)
+{
+    if (!c) return LTJK_EINVAL;
+    c->resident_req = enable != 0;
     return LTJK_OK;
 }
 

@@ -109,7 +109,9 @@ struct PWork {              // one digestion work record: a matrix A(c, m) = bas
     int rlist;              // K: offset of the row partner list in pl_ao;           J: offset into jrow (rows)
     int tile0;              // first entry of this record in the tile-prefix array (contraction length per row tile)
     int ntiles;
-    int pad;
+    int orient;             // 1: rows contiguous in storage;  2: the mirrored role assignment, A tile gathered.
+                            // Orientation 2 (K): rows (c,iy) with c from the partner list of X (rlist), contraction r
+                            // from the partner list of Y (clist), one pass per component ix.  (J): rows q, contraction p.
 };
 
 struct PChunk {
@@ -181,6 +183,8 @@ struct ltjk_ctx {
     long long pring_half = 0;              // doubles per half
     int* d_pcounter = nullptr;             // work-stealing cursors, one per digestion launch of a build
     int pcounter_next = 0, pcounter_cap = 0;
+    bool resident_req = false;             // keep all integral panels of the geometry in HBM across builds (strategy 1)
+    bool resident = false, panels_valid = false;
     int digest_mode_req = 0;               // requested: 0 = auto, 1 = block panels (dense), 2 = pair lists
     int digest_mode = 1;                   // in use: 1 = block panels, 2 = pair lists (screening-aware)
     bool have_pl = false;

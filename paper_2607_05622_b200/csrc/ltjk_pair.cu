@@ -160,6 +160,9 @@ int build_pairlists(ltjk_ctx* c)
                         if (ra == rb) continue;
                         const double qrmax = h.sl_q[ra];
                         if (qcmax * qrmax < tau) continue;
+                        // one block per mirrored pair (X,Y,g2,g4) <-> (Y,X,g4,g2): the mirror image is digested
+                        // through orientation 2 of the stored block
+                        if (!(X > Y || (X == Y && g2 >= g4))) continue;
                         const int Lc = count_ao(h, X, g2, qrmax, tau), Lr = count_ao(h, Y, g4, qcmax, tau);
                         if (Lc == 0 || Lr == 0) continue;
                         const long long ci = chunk_index(gp_index(h.sh_grp[X], g2), gp_index(h.sh_grp[Y], g4));
@@ -223,10 +226,7 @@ int build_pairlists(ltjk_ctx* c)
                 if (np > 0 && nq > 0) {
                     ch.j0_lda = (int)((np + 1) & ~1ll);
                     ch.j0_off = used; used += (long long)ch.j0_lda * nq;           // rows (gab), contraction (gcd)
-                    if (P != Q) {
-                        ch.j1_lda = (int)((nq + 1) & ~1ll);
-                        ch.j1_off = used; used += (long long)ch.j1_lda * np;       // rows (gcd), contraction (gab)
-                    }
+                    // off-diagonal chunks: rows (gcd) x contraction (gab) is orientation 2 of the same array
                 }
                 ch.doubles = used;
                 maxchunk = std::max(maxchunk, used);
@@ -253,36 +253,54 @@ int build_pairlists(ltjk_ctx* c)
                     const PBlock& b = blk[(((size_t)X * ns + Y) * G + g2) * G + g4];
                     if (b.off < 0) continue;
                     const int nX = h.ncomp[X], nY = h.ncomp[Y];
-                    PWork w = PWork();
-                    w.off = b.off; w.lda = (int)(((long long)nX * b.Lr + 1) & ~1ll);
-                    w.nrows = nX * b.Lr; w.kind = 0; w.nY = nY; w.Lc = b.Lc; w.x0 = h.ao0[X]; w.nX = nX; w.y0 = h.ao0[Y];
-                    w.clist = h.pl_start[X * G + g2]; w.rlist = h.pl_start[Y * G + g4];
-                    w.tile0 = (int)tiles.size();
-                    w.ntiles = (w.nrows + kDigestRows - 1) / kDigestRows;
-                    double cost = 0.0;
-                    for (int t = 0; t < w.ntiles; ++t) {
-                        const int r0 = (t * kDigestRows) / nX;                 // smallest row rank of the tile = largest Q
-                        const double qr = q_at_rank(h, Y, g4, r0);
-                        const int lc = std::min(b.Lc, count_ao(h, X, g2, qr, tau));
-                        tiles.push_back(lc);
-                        cost += (double)((lc + 15) / 16);
-                    }
                     PChunk& ch = chunks[chunk_pos(gp_index(h.sh_grp[X], g2), gp_index(h.sh_grp[Y], g4))];
-                    ch.exec_rows_chunks_K += cost * nY * kDigestRows * 16.0;
-                    cworkK[chunk_pos(gp_index(h.sh_grp[X], g2), gp_index(h.sh_grp[Y], g4))].push_back(w);
+                    std::vector<PWork>& dst = cworkK[chunk_pos(gp_index(h.sh_grp[X], g2), gp_index(h.sh_grp[Y], g4))];
+                    const bool self = (X == Y && g2 == g4);        // its own mirror image: orientation 1 covers it
+                    for (int orient = 1; orient <= (self ? 1 : 2); ++orient) {
+                        PWork w = PWork();
+                        w.off = b.off; w.lda = (int)(((long long)nX * b.Lr + 1) & ~1ll);
+                        w.kind = 0; w.orient = orient; w.nY = nY; w.Lc = b.Lc; w.x0 = h.ao0[X]; w.nX = nX; w.y0 = h.ao0[Y];
+                        w.tile0 = (int)tiles.size();
+                        double cost = 0.0;
+                        if (orient == 1) {
+                            w.nrows = nX * b.Lr;
+                            w.clist = h.pl_start[X * G + g2]; w.rlist = h.pl_start[Y * G + g4];
+                            w.ntiles = (w.nrows + kDigestRows - 1) / kDigestRows;
+                            for (int t = 0; t < w.ntiles; ++t) {
+                                const int r0 = (t * kDigestRows) / nX;         // smallest row rank of the tile = largest Q
+                                const int lc = std::min(b.Lc, count_ao(h, X, g2, q_at_rank(h, Y, g4, r0), tau));
+                                tiles.push_back(lc);
+                                cost += (double)((lc + 15) / 16);
+                            }
+                            cost *= nY;
+                        } else {
+                            w.nrows = nY * b.Lc;
+                            w.clist = h.pl_start[Y * G + g4]; w.rlist = h.pl_start[X * G + g2];
+                            w.ntiles = (w.nrows + kDigestRows - 1) / kDigestRows;
+                            for (int t = 0; t < w.ntiles; ++t) {
+                                const int c0 = (t * kDigestRows) / nY;
+                                const int lr = std::min(b.Lr, count_ao(h, Y, g4, q_at_rank(h, X, g2, c0), tau));
+                                tiles.push_back(lr);
+                                cost += (double)((lr * nX + 15) / 16);     // contraction over (r, ix) jointly
+                            }
+                        }
+                        ch.exec_rows_chunks_K += cost * kDigestRows * 16.0;
+                        dst.push_back(w);
+                    }
                 }
     for (size_t ci = 0; ci < chunks.size(); ++ci) {
         PChunk& ch = chunks[ci];
-        for (int which = 0; which < 2; ++which) {
-            const long long joff = which == 0 ? ch.j0_off : ch.j1_off;
-            if (joff < 0) continue;
-            const int lda = which == 0 ? ch.j0_lda : ch.j1_lda;
-            const int gpr = which == 0 ? ch.gab : ch.gcd, gpc = which == 0 ? ch.gcd : ch.gab;
+        if (ch.j0_off < 0) continue;
+        // the J array of the chunk: element (contraction q of gcd, row p of gab) at j0[q * lda + p].  Orientation 1:
+        // rows p, contraction q;  orientation 2 (off-diagonal chunks only): rows q, contraction p (row-major reads).
+        for (int orient = 1; orient <= (ch.gab == ch.gcd ? 1 : 2); ++orient) {
+            const int lda = ch.j0_lda;
+            const int gpr = orient == 1 ? ch.gab : ch.gcd, gpc = orient == 1 ? ch.gcd : ch.gab;
             const long long nr = jrow_start[gpr + 1] - jrow_start[gpr], ncn = jrow_start[gpc + 1] - jrow_start[gpc];
             const double* qr = jq.data() + jrow_start[gpr];
             const double* qc = jq.data() + jrow_start[gpc];
             // one record per row tile and contraction slice of <= kJSlice columns: J records would otherwise be the
-            // long pole of the launch (a row tile contracts over every significant ket pair of the chunk)
+            // long pole of the launch (a row tile contracts over every significant pair of the other side)
             const long long kJSlice = 2048;
             for (long long m0 = 0; m0 < nr; m0 += kDigestRows) {
                 const double qrow = qr[m0];
@@ -290,9 +308,10 @@ int build_pairlists(ltjk_ctx* c)
                 while (lo < hi) { const long long mid = (lo + hi) / 2; if (qc[mid] * qrow >= tau) lo = mid + 1; else hi = mid; }
                 for (long long c0 = 0; c0 < lo; c0 += kJSlice) {
                     PWork w = PWork();
-                    w.off = joff + m0 + c0 * lda; w.lda = lda;
+                    w.off = orient == 1 ? ch.j0_off + m0 + c0 * lda : ch.j0_off + m0 * lda + c0;
+                    w.lda = lda;
                     w.nrows = (int)std::min<long long>(kDigestRows, nr - m0);
-                    w.kind = 1; w.nY = 1; w.Lc = 0; w.x0 = 0; w.nX = 1; w.y0 = 0;
+                    w.kind = 1; w.orient = orient; w.nY = 1; w.Lc = 0; w.x0 = 0; w.nX = 1; w.y0 = 0;
                     w.clist = (int)(jrow_start[gpc] + c0); w.rlist = (int)(jrow_start[gpr] + m0);
                     w.tile0 = (int)tiles.size();
                     w.ntiles = 1;
@@ -309,7 +328,7 @@ int build_pairlists(ltjk_ctx* c)
     auto cost_of = [&](const PWork& w) {
         double s = 0.0;
         for (int t = 0; t < w.ntiles; ++t) s += (double)((tiles[w.tile0 + t] + 15) / 16);
-        return s * w.nY;
+        return s * (w.kind ? 1 : (w.orient == 1 ? w.nY : w.nX));   // (orientation 2: upper estimate)
     };
     int nbuf = 0;
     long long maxchunk = 0;

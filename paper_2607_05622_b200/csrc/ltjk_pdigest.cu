@@ -90,28 +90,48 @@ __global__ void __launch_bounds__(kDigestThreads, 1) pdigest_kernel(const PDiges
             const PWork wk = g.work[wi];
             const double* __restrict__ Bmat = wk.kind ? g.Dst : g.Dt;
             const int* __restrict__ clist = (wk.kind ? g.jrow : g.pl_ao) + wk.clist;
+            // orientation 2 of a K block contracts over (r, ix) jointly: kappa = r * nX + ix is contiguous in storage
+            const bool k2 = !wk.kind && wk.orient == 2;
+            const int npass = (!wk.kind && wk.orient == 1) ? wk.nY : 1;
             for (int t = 0; t < wk.ntiles; ++t) {
-                const int lc = g.tiles[wk.tile0 + t];
+                const int lc = g.tiles[wk.tile0 + t] * (k2 ? wk.nX : 1);
                 const int nch = (lc + kKC - 1) / kKC;
                 const int nrows_t = min(kMT, wk.nrows - t * kMT);
+                // orientation 2: producer thread pt gathers row t*128 + pt of the tile (16 consecutive doubles per chunk)
+                long long rowbase = -1;
+                if (wk.orient == 2 && pt < nrows_t) {
+                    const int m = t * kMT + pt;
+                    rowbase = wk.kind ? (long long)m * wk.lda : ((long long)(m % wk.nY) * wk.Lc + m / wk.nY) * wk.lda;
+                }
                 for (int cb = 0; cb < g.ncolblk; ++cb) {
                     const int n0 = cb * 32 * TN;
-                    for (int iy = 0; iy < wk.nY; ++iy) {
-                        const double* __restrict__ Ab = g.ring + wk.off + (long long)iy * wk.Lc * wk.lda;
+                    for (int ip = 0; ip < npass; ++ip) {
+                        const double* __restrict__ Ab = g.ring + wk.off + (long long)ip * wk.Lc * wk.lda;
+                        // B row of contraction index c: orientation 1: D[c_ao][y0 + iy];  2: D[r_ao][x0 + ix];  J: Ds[pair]
+                        const int bfix = wk.y0 + ip;
                         for (int ch = 0; ch < nch; ++ch, ++gch) {
                             const int st = gch % kStages;
                             if (gch >= kStages) mbar_wait(&S.empty[st], (unsigned)((gch / kStages - 1) & 1));
-                            // A tile: 16 contraction rows of 128 doubles = 1024 pieces of 16 bytes, 8 per thread
+                            if (wk.orient == 1) {
+                                // A tile: 16 contraction rows of 128 doubles = 1024 pieces of 16 bytes, 8 per thread
 #pragma unroll
-                            for (int j = 0; j < (kKC * kMT / 2) / kProducerThreads; ++j) {
-                                const int piece = pt + kProducerThreads * j;
-                                const int k = piece >> 6, pc = piece & 63;
-                                const int c = ch * kKC + k;
-                                int bytes = (nrows_t - 2 * pc) * 8;
-                                bytes = (c < lc) ? max(0, min(16, bytes)) : 0;
-                                const double* src = bytes ? (Ab + (long long)c * wk.lda + t * kMT + 2 * pc) : g.ring;
-                                const unsigned s = (unsigned)__cvta_generic_to_shared(&S.A[st][k][2 * pc]);
-                                asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(src), "r"(bytes));
+                                for (int j = 0; j < (kKC * kMT / 2) / kProducerThreads; ++j) {
+                                    const int piece = pt + kProducerThreads * j;
+                                    const int k = piece >> 6, pc = piece & 63;
+                                    const int c = ch * kKC + k;
+                                    int bytes = (nrows_t - 2 * pc) * 8;
+                                    bytes = (c < lc) ? max(0, min(16, bytes)) : 0;
+                                    const double* src = bytes ? (Ab + (long long)c * wk.lda + t * kMT + 2 * pc) : g.ring;
+                                    const unsigned sa = (unsigned)__cvta_generic_to_shared(&S.A[st][k][2 * pc]);
+                                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(src), "r"(bytes));
+                                }
+                            } else {
+#pragma unroll 4
+                                for (int k = 0; k < kKC; ++k) {
+                                    const int c = ch * kKC + k;
+                                    const bool ok = (rowbase >= 0) && (c < lc);
+                                    cp_async8(&S.A[st][k][pt], ok ? (Ab + rowbase + c) : g.ring, ok);
+                                }
                             }
                             // B tile: kKC gathered density rows of 32 TN doubles; warp pw copies rows pw, pw+4, ...
 #pragma unroll
@@ -119,7 +139,11 @@ __global__ void __launch_bounds__(kDigestThreads, 1) pdigest_kernel(const PDiges
                                 const int k = pw + kProducerWarps * h, c = ch * kKC + k;
                                 const bool ok = c < lc;
                                 long long brow = 0;
-                                if (ok) brow = wk.kind ? (long long)clist[c] : (long long)clist[c] * N + wk.y0 + iy;
+                                if (ok) {
+                                    if (wk.kind) brow = (long long)clist[c];
+                                    else if (k2) brow = (long long)clist[c / wk.nX] * N + wk.x0 + c % wk.nX;
+                                    else brow = (long long)clist[c] * N + bfix;
+                                }
                                 const double* src = Bmat + brow * nDp + n0;
                                 for (int pc = lane; pc < 16 * TN; pc += 32)
                                     cp_async16(&S.B[st][k][pc * 2], src + (ok ? pc * 2 : 0), ok);
@@ -157,8 +181,10 @@ __global__ void __launch_bounds__(kDigestThreads, 1) pdigest_kernel(const PDiges
         double* __restrict__ Out = wk.kind ? g.Jt : g.Kt;
         const int* __restrict__ rlist = (wk.kind ? g.jrow : g.pl_ao) + wk.rlist;
         for (int t = 0; t < wk.ntiles; ++t) {
-            const int lc = g.tiles[wk.tile0 + t];
-            const int nch = ((lc + kKC - 1) / kKC) * wk.nY;       // one accumulation over all components of Y
+            const bool k2 = !wk.kind && wk.orient == 2;
+            const int lc = g.tiles[wk.tile0 + t] * (k2 ? wk.nX : 1);
+            // one accumulation over all passes (components of Y in orientation 1)
+            const int nch = ((lc + kKC - 1) / kKC) * ((!wk.kind && wk.orient == 1) ? wk.nY : 1);
             if (nch == 0) continue;
             const bool warp_active = t * kMT + wrow < wk.nrows;
             // output rows of this thread: looked up before the contraction so that the flush does not wait on them
@@ -167,7 +193,11 @@ __global__ void __launch_bounds__(kDigestThreads, 1) pdigest_kernel(const PDiges
             for (int r = 0; r < kRows; ++r) {
                 const int m = t * kMT + trow + r;
                 orow[r] = -1;
-                if (m < wk.nrows) orow[r] = wk.kind ? rlist[m] : (wk.x0 + m % wk.nX) * N + rlist[m / wk.nX];
+                if (m < wk.nrows) {
+                    if (wk.kind) orow[r] = rlist[m];
+                    else if (wk.orient == 1) orow[r] = (wk.x0 + m % wk.nX) * N + rlist[m / wk.nX];     // K[x][r]
+                    else orow[r] = (wk.y0 + m % wk.nY) * N + rlist[m / wk.nY];                          // K[y][c]
+                }
             }
             for (int cb = 0; cb < g.ncolblk; ++cb) {
                 const int n0 = cb * 32 * TN;
@@ -294,12 +324,22 @@ __global__ void __launch_bounds__(128) pzero_kernel(const PZeroArgs g)
         const double* __restrict__ qr = (wk.kind ? g.jq : g.pl_q) + wk.rlist;
         for (int m = threadIdx.x; m < wk.nrows; m += blockDim.x) {
             const int lc = g.tiles[wk.tile0 + m / kDigestRows];
-            const double qrow = qr[wk.kind ? m : m / wk.nX];
+            const int rdiv = wk.kind ? 1 : (wk.orient == 1 ? wk.nX : wk.nY);
+            const double qrow = qr[m / rdiv];
             int lo = 0, hi = lc;                                  // first contraction index with Q * Q_row < tau
             while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] * qrow >= g.tau) lo = mid + 1; else hi = mid; }
-            for (int iy = 0; iy < wk.nY; ++iy) {
-                double* __restrict__ A = g.ring + wk.off + (long long)iy * wk.Lc * wk.lda + m;
-                for (int cidx = lo; cidx < lc; ++cidx) A[(long long)cidx * wk.lda] = 0.0;
+            if (wk.orient == 1) {
+                for (int iy = 0; iy < wk.nY; ++iy) {
+                    double* __restrict__ A = g.ring + wk.off + (long long)iy * wk.Lc * wk.lda + m;
+                    for (int cidx = lo; cidx < lc; ++cidx) A[(long long)cidx * wk.lda] = 0.0;
+                }
+            } else if (wk.kind) {
+                double* __restrict__ A = g.ring + wk.off + (long long)m * wk.lda;
+                for (int cidx = lo; cidx < lc; ++cidx) A[cidx] = 0.0;
+            } else {
+                double* __restrict__ A = g.ring + wk.off + ((long long)(m % wk.nY) * wk.Lc + m / wk.nY) * wk.lda;
+                for (int cidx = lo; cidx < lc; ++cidx)
+                    for (int ix = 0; ix < wk.nX; ++ix) A[(long long)cidx * wk.nX + ix] = 0.0;
             }
         }
     }

@@ -5,7 +5,8 @@
 // (bra b, ket k) evaluates the unique quartet (AB|CD) when Q_AB Q_CD >= tau (reading A9) and
 // returns at once otherwise ("only the realised buckets are launched").  Each value (ij|kl) is stored
 // under its eight role assignments (x,c,y,r) -- the eight permutational images of Eq. 25 (reading
-// A5) -- at  T_{XY}[iy][rank_x(c)][rank_y(r)][ix]  and twice, with the shell-level fold weight, in the J arrays.
+// A5) -- at  T_{XY}[iy][rank_x(c)][rank_y(r)][ix]; of every mirrored pair of assignments (x,c,y,r) <-> (y,r,x,c) only
+// the block with X >= Y exists (the digestion reads it in two orientations), so 4 K stores and 1 J store per value.
 #include "ltjk_internal.h"
 #include "eri_core.h"
 
@@ -35,6 +36,7 @@ __device__ __forceinline__ void store_copy(const PEriArgs& g, const int* sh, con
     const int ns = g.t.nshell, G = g.pl.G;
     const int X = sh[PX], C = sh[PC], Y = sh[PY], R = sh[PR];
     const PBlock b = g.pl.blk[(((size_t)X * ns + Y) * G + g.pl.sh_grp[C]) * G + g.pl.sh_grp[R]];
+    if (b.off < 0) return;          // the mirrored role assignment owns the block (digested through orientation 2)
     const int pc = g.pl.pos[(size_t)X * ns + C] + org[PC], pr = g.pl.pos[(size_t)Y * ns + R] + org[PR];
     constexpr int NX = ncomp[PX];
     const long long ldr = ((long long)NX * b.Lr + 1) & ~1ll;
@@ -100,8 +102,8 @@ __device__ __forceinline__ void store_all(const PEriArgs& g, const PPair& P1, co
                 for (int d = 0; d < ED; ++d) {
                     const long long q = P2.joff + cc * ND + d;
                     const double val = w * v[((a * EB + b) * EC + cc) * ED + d];
-                    JA[q * g.jA_lda + p] = val;
-                    if (pq || g.jA_off != g.jB_off) JB[p * g.jB_lda + q] = val;
+                    if (g.jA_off >= 0) JA[q * g.jA_lda + p] = val;
+                    if (g.jB_off >= 0 && (pq || g.jA_off != g.jB_off)) JB[p * g.jB_lda + q] = val;
                 }
         }
 }
@@ -295,9 +297,11 @@ int launch_peri_chunk(ltjk_ctx* c, const PChunk& ch)
                 g.bra = c->d_ppairs + b0; g.nbra = (int)bn;
                 g.ket = c->d_ppairs + k0; g.nket = (int)kn;
                 g.diag = (ch.gab == ch.gcd && cb == ck) ? 1 : 0;
+                // the chunk's J array j0[q(gcd) * lda + p(gab)]: diagonal chunks hold both triangles; off the diagonal the
+                // bra pair is the row p (no swap) or the contraction index q (swapped launch)
                 if (ch.gab == ch.gcd) { g.jA_off = ch.j0_off; g.jA_lda = ch.j0_lda; g.jB_off = ch.j0_off; g.jB_lda = ch.j0_lda; }
-                else if (!swap) { g.jA_off = ch.j0_off; g.jA_lda = ch.j0_lda; g.jB_off = ch.j1_off; g.jB_lda = ch.j1_lda; }
-                else { g.jA_off = ch.j1_off; g.jA_lda = ch.j1_lda; g.jB_off = ch.j0_off; g.jB_lda = ch.j0_lda; }
+                else if (!swap) { g.jA_off = ch.j0_off; g.jA_lda = ch.j0_lda; g.jB_off = -1; g.jB_lda = 0; }
+                else { g.jA_off = -1; g.jA_lda = 0; g.jB_off = ch.j0_off; g.jB_lda = ch.j0_lda; }
                 if (g.nbra > 65535) return set_err(c, LTJK_EINVAL, "internal: bra pair list exceeds the launch grid");
                 c->st_launches++;
                 int rc;

@@ -476,3 +476,31 @@ def test_level2_density_from_laplace_fock(torch_cuda, tiny):
     assert relerr(F.cpu().numpy(), Fr) < TOL
     assert relerr(D2.cpu().numpy().reshape(-1, N, N), D2r.reshape(-1, N, N)) < TOL
     assert np.abs(D2r).max() > 0
+
+
+def test_resident_panels_reused_across_builds(torch_cuda, small):
+    """ltjk_set_resident: the integral panels of the geometry are generated by the first build and only digested by
+    later ones (no ERI launches); results stay those of the integral-direct path, for new densities and batch sizes."""
+    from paper_2607_05622_b200 import ltjk
+    torch = torch_cuda
+    w = small
+    ctx = ltjk.Context(0)
+    ctx.set_digest_mode(1)
+    ctx.set_resident(True)
+    ctx.set_basis(w.basis)
+    ctx.build_shell_pairs(w.schwarz_tau)
+    D = random_densities(w.nao, 40, seed=51)
+    Jr, Kr, _ = O.jk_folded(w.basis, D[[0, 7, 39]], w.schwarz_tau)
+    J1, K1 = gpu_jk(torch, ctx, D[:8])
+    n_first = ctx.get_stats()["n_launches"]
+    J2, K2 = gpu_jk(torch, ctx, D)                       # second build: other densities, other column blocking
+    n_second = ctx.get_stats()["n_launches"]
+    assert n_second < n_first                             # no ERI launches any more
+    assert relerr(J1[[0, 7]], Jr[:2]) < TOL and relerr(K1[[0, 7]], Kr[:2]) < TOL
+    assert relerr(J2[[0, 7, 39]], Jr) < TOL and relerr(K2[[0, 7, 39]], Kr) < TOL
+    # a new geometry invalidates the cache
+    ctx.set_basis(w.basis)
+    ctx.build_shell_pairs(w.schwarz_tau)
+    J3, K3 = gpu_jk(torch, ctx, D[:8])
+    assert ctx.get_stats()["n_launches"] == n_first
+    assert relerr(K3[[0, 7]], Kr[:2]) < TOL
