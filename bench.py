@@ -184,7 +184,8 @@ def run_reference(args, rank, world):
     print(json.dumps(out), flush=True)
 
 
-def sweep_report(torch, ltjk, w, local, T_host, steps, warmup, world, barrier, max_over_ranks, want_e2e=True, mode=0):
+def sweep_report(torch, ltjk, w, local, T_host, steps, warmup, world, barrier, max_over_ranks, want_e2e=True, mode=0,
+                 shard=None):
     """Set up one workload (geometry-frozen part outside the timed region), time `steps` whole sweeps with CUDA events
     on the ctx stream, then the per-phase split (timing mode) and the roofline of the digestion kernel."""
     N, nD = w.nao, w.nD
@@ -199,12 +200,25 @@ def sweep_report(torch, ltjk, w, local, T_host, steps, warmup, world, barrier, m
     Co, Cv, eo, ev, Td = dev(w.C_occ), dev(w.C_vir), dev(w.eps_occ), dev(w.eps_vir), dev(T_host)
     D = torch.empty((w.ntau, w.nT, N, N), dtype=torch.float64, device="cuda")
     Dn = D.view(nD, N, N)
-    J = torch.empty_like(Dn)
-    K = torch.empty_like(Dn)
+    if shard is None:
+        J = torch.empty_like(Dn)
+        K = torch.empty_like(Dn)
 
-    def step():
-        ctx.build_pseudo_densities(Co, Cv, eo, ev, Td, tau, D)
-        ctx.jk_build(Dn, J, K)
+        def step():
+            ctx.build_pseudo_densities(Co, Cv, eo, ev, Td, tau, D)
+            ctx.jk_build(Dn, J, K)
+    else:
+        # ONE sweep split over the ranks: this rank builds densities shard = rank::world of the sweep
+        idx = torch.from_numpy(np.ascontiguousarray(shard)).cuda()
+        Ds = torch.empty((len(shard), N, N), dtype=torch.float64, device="cuda")
+        J = torch.empty_like(Ds)
+        K = torch.empty_like(Ds)
+
+        def step():
+            ctx.build_pseudo_densities(Co, Cv, eo, ev, Td, tau, D)
+            torch.index_select(Dn, 0, idx, out=Ds)
+            ctx.jk_build(Ds, J, K)
+        want_e2e = False
 
     for _ in range(warmup):
         step()
@@ -217,7 +231,7 @@ def sweep_report(torch, ltjk, w, local, T_host, steps, warmup, world, barrier, m
     e1.record(stream)
     barrier()
     ms_per_step = max_over_ranks(e0.elapsed_time(e1), "cuda") / steps
-    rep = {"ctx": ctx, "tau": tau, "Dn": Dn, "J": J, "K": K, "ms_per_step": ms_per_step, "nq_kept": nq_kept,
+    rep = {"ctx": ctx, "tau": tau, "Dn": Dn if shard is None else Ds, "J": J, "K": K, "ms_per_step": ms_per_step, "nq_kept": nq_kept,
            "launches_per_step": ctx.get_stats()["n_launches"] + 3, "laplace_maxerr": lap_err,
            "digest_mode": ctx.get_digest_mode()}
 
@@ -262,7 +276,7 @@ def roofline_of(torch, ctx, w, rep, peak_tf):
     ctx.set_timing(False)
     Q = ctx.get_schwarz()
     ints = kept_integrals(Q, w.basis.l, w.schwarz_tau)
-    alg = 20.0 * w.nD * ints                 # 2 J + 8 K FMAs per unique integral and density
+    alg = 20.0 * Dn.shape[0] * ints          # 2 J + 8 K FMAs per unique integral and density
     achieved = alg / (st["digest_ms"] * 1e-3) / 1e12
     return {"bound": "alu",
             "kernel": "digest kernel (J/K digestion; achieved = algorithmic flop of one sweep / summed duration of its launches)",
@@ -292,6 +306,8 @@ def main():
     ap.add_argument("--impl", default="ltjk")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mode", type=int, default=0, help="digestion strategy (ltjk_set_digest_mode): 0 auto, 1 panels, 2 pair lists")
+    ap.add_argument("--shard", choices=["problems", "densities"], default="problems",
+                    help="N > 1: every rank its own sweep (weak scaling, default) or ONE sweep's densities dealt round-robin (strong)")
     ap.add_argument("--no-large", action="store_true", help="skip the 730-AO sub-run reported under config.large_730")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
@@ -323,8 +339,11 @@ def main():
     N, nD = w.nao, w.nD
     # Multi-GPU: the path shards over independent problems -- every rank runs its own
     # sweep on its own batch of n_T amplitude sets (same molecule, rank-seeded T); no data-path collective.
-    from paper_2607_05622_b200.dist import max_over_ranks, rank_amplitudes, whole_job_builds_per_s
-    T_host = rank_amplitudes(w, rank)
+    from paper_2607_05622_b200.dist import (density_shard, max_over_ranks, rank_amplitudes, sharded_sweep_builds_per_s,
+                                            whole_job_builds_per_s)
+    strong = world > 1 and args.shard == "densities"
+    T_host = w.T if strong else rank_amplitudes(w, rank)
+    shard = density_shard(nD, rank, world) if strong else None
 
     def barrier():
         if world > 1:
@@ -334,10 +353,11 @@ def main():
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    rep = sweep_report(torch, ltjk, w, local, T_host, args.steps, args.warmup, world, barrier, max_over_ranks, mode=args.mode)
+    rep = sweep_report(torch, ltjk, w, local, T_host, args.steps, args.warmup, world, barrier, max_over_ranks, mode=args.mode,
+                       shard=shard)
     clocks = sampler.stop() if rank == 0 else None
     ms_per_step = rep["ms_per_step"]
-    value = whole_job_builds_per_s(nD, world, ms_per_step)
+    value = sharded_sweep_builds_per_s(nD, ms_per_step) if strong else whole_job_builds_per_s(nD, world, ms_per_step)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -372,8 +392,10 @@ def main():
     if not args.no_cpu_baseline:
         cpu = oracle_sample(w, Dn.cpu().numpy(), target_s=20.0)
     launches = int(rep["launches_per_step"] * args.steps)
-    e2e = {"value": whole_job_builds_per_s(nD, world, rep["ms_e2e"]), "unit": UNIT, "h2d_bytes_per_step": rep["h2d"],
-           "d2h_bytes_per_step": rep["d2h"], "ms_per_step": rep["ms_e2e"]}
+    e2e = None
+    if "ms_e2e" in rep:
+        e2e = {"value": whole_job_builds_per_s(nD, world, rep["ms_e2e"]), "unit": UNIT, "h2d_bytes_per_step": rep["h2d"],
+               "d2h_bytes_per_step": rep["d2h"], "ms_per_step": rep["ms_e2e"]}
     config = {"workload": "%s (%d AO, %d atoms, n_tau=%d x n_T=%d = %d non-symmetric densities per sweep)" %
                           (w.name, N, w.basis.natom, w.ntau, w.nT, nD),
               "tau_schwarz": w.schwarz_tau, "shell_quartets_kept": rep["nq_kept"], "unique_integrals_kept": ints,
@@ -443,7 +465,7 @@ def main():
         launches += int(repl["launches_per_step"] * 2)
         repl["ctx"].close()
     out = {"metric": metric_name(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+           "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if strong else "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config, "clocks": clocks, "e2e": e2e,
            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(out), flush=True)

@@ -5,6 +5,12 @@
 * O9 minimax Laplace grid by Remez exchange + Newton in 120-digit arithmetic       PAPER.md:L126 Eq. (11)
 * O10 pseudo-density as explicit loops                                            PAPER.md:L136-145 Eqs. (13),(15)
 
+* N1 laplace_fock / laplace_accumulate (Eqs. (19), (21)), N3 pp_ladder
+
+Pins (tests/test_oracle_*.py, CPU tier): O9 equi-oscillation certificate, scaling law, Lawson cross-check; O10 tau = 0
+product, rank-1 Eq. (14) case, unit amplitudes, layout, denominator resolution with the golden grid; N1 C = I, K = 2J,
+rectangular C; N3 one-centre closed form, loops, bra-ket symmetry, AO-direct K route.  Nothing is "parity unpinned".
+
 Nothing here imports the CUDA package except the shared, arithmetic-free input generators.
 """
 from __future__ import annotations
