@@ -14,7 +14,9 @@
  *     memory the caller must free.  Internal device buffers belong to the context.
  *   - All device work is enqueued on the context's stream; calls that launch kernels return without
  *     synchronising (the caller syncs through its own stream API) unless stated otherwise.
- *   - A context is not thread-safe.
+ *   - A context is not thread-safe.  Calls that touch the device make the context's device the calling thread's
+ *     current CUDA device and leave it so; ltjk_create also raises the release threshold of that device's default
+ *     stream-ordered memory pool so that the library's scratch allocations are reused between calls.
  *   - There is NO CPU fallback: without a CUDA device ltjk_create fails with LTJK_ECUDA.
  *   - Units: bohr, hartree (PAPER.md reports E_h/a_0 throughout, e.g. L450).
  *   - No prefactor is embedded anywhere: no w_alpha, no exchange 1/2, no spin factor 2

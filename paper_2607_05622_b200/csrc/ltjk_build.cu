@@ -58,6 +58,11 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     // ---- a1: basis to the device (temporary, caller order) and a2: pair records + Schwarz bounds
     double *d_xyz = nullptr, *d_exps = nullptr, *d_coef = nullptr;
     int *d_atom = nullptr, *d_l = nullptr, *d_nprim = nullptr, *d_poff = nullptr, *d_i2e = nullptr;
+    struct TmpGuard {          // the temporary basis copies are released on every exit path
+        void** p[8];
+        ~TmpGuard() { for (void** q : p) if (*q) { cudaFree(*q); *q = nullptr; } }
+    } guard{{(void**)&d_xyz, (void**)&d_exps, (void**)&d_coef, (void**)&d_atom, (void**)&d_l, (void**)&d_nprim,
+             (void**)&d_poff, (void**)&d_i2e}};
     int rc;
     if ((rc = upload(c, &d_xyz, c->xyz)) || (rc = upload(c, &d_exps, c->exps)) || (rc = upload(c, &d_coef, c->coef)) ||
         (rc = upload(c, &d_atom, c->atom)) || (rc = upload(c, &d_l, c->l)) || (rc = upload(c, &d_nprim, c->nprim)) ||
@@ -78,8 +83,7 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     LTJK_CUDA(c, cudaMemcpyAsync(c->Qhost.data(), t.schwarz, sizeof(double) * (size_t)ns * ns, cudaMemcpyDeviceToHost,
                                  c->stream));
     LTJK_CUDA(c, cudaStreamSynchronize(c->stream));
-    cudaFree(d_xyz); cudaFree(d_exps); cudaFree(d_coef); cudaFree(d_atom); cudaFree(d_l); cudaFree(d_nprim);
-    cudaFree(d_poff); cudaFree(d_i2e);
+    guard.~TmpGuard();      // early release (idempotent: the pointers are nulled)
 
     // ---- a5: screened quartet count (canonical, shell level): #{(p,q): p >= q, Q_p Q_q >= tau}
     {

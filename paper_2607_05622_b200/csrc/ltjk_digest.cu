@@ -329,15 +329,13 @@ template <int TN>
 static int launch_digest_tn(ltjk_ctx* c, const DigestArgs& g, int nitems, int ncolblk)
 {
     const size_t smem = sizeof(DigestSmem<TN>);
-    static bool attr_set = false;
-    if (!attr_set) {
-        LTJK_CUDA(c, cudaFuncSetAttribute(digest_kernel<TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    // per launch: the attribute belongs to the device's context, and a process may hold contexts on several devices
+    LTJK_CUDA(c, cudaFuncSetAttribute(digest_kernel<TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     const long long nvirt = (long long)nitems * ncolblk;
+    if (nvirt > 0x7fffffffll) return set_err(c, LTJK_EINVAL, "digest: more than 2^31 work items in one launch");
     // 32 persistent waves (measured 2..64 on B200: 632, 626, 621, 609, 601, 598 ms of digestion per 439-AO sweep):
     // the hardware block scheduler balances the load, each CTA still prefetches across its items
     const int grid = (int)std::min<long long>(nvirt, 32ll * nsm);

@@ -291,12 +291,8 @@ static int launch_cls(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
         if constexpr (lb[CB] > 0 && lb[CK] > 0 && V::NE * V::NF >= 128) {
             constexpr int QS = V::NE * V::NF + ltjk_gen::Hrr<la[CB], lb[CB]>::NAB * V::NF;
             constexpr int smem = (kCoopThreads / 16) * QS * (int)sizeof(double);
-            static bool attr = false;
-            if (!attr) {
-                LTJK_CUDA(c, cudaFuncSetAttribute(eri_panel_coop_kernel<la[CB], lb[CB], la[CK], lb[CK]>,
-                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-                attr = true;
-            }
+            LTJK_CUDA(c, cudaFuncSetAttribute(eri_panel_coop_kernel<la[CB], lb[CB], la[CK], lb[CK]>,
+                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
             const long long nq = (long long)maxkets * g.qn;
             const int per = kCoopThreads / 16;
             eri_panel_coop_kernel<la[CB], lb[CB], la[CK], lb[CK]>
@@ -306,12 +302,9 @@ static int launch_cls(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
         }
         const long long nthr = (long long)maxkets * g.qn;
         const int bs = 64;
-        static bool carve = false;      // no shared memory used: give the whole unified cache to L1 (local-memory spills)
-        if (!carve) {
-            cudaFuncSetAttribute(eri_panel_kernel<la[CB], lb[CB], la[CK], lb[CK]>,
-                                 cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxL1);
-            carve = true;
-        }
+        // no shared memory used: give the whole unified cache to L1 (local-memory spills)
+        cudaFuncSetAttribute(eri_panel_kernel<la[CB], lb[CB], la[CK], lb[CK]>,
+                             cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxL1);
         eri_panel_kernel<la[CB], lb[CB], la[CK], lb[CK]>
             <<<dim3((unsigned)((nthr + bs - 1) / bs), nsub), bs, 0, c->eri_stream>>>(g);
         LTJK_CUDA(c, cudaGetLastError());

@@ -31,9 +31,12 @@ struct PDigestArgs {
     int* counter;          // work-stealing cursor of this launch (zeroed by the host)
 };
 
+constexpr int kRowPitch = kKC + 2;      // orientation 2: row-major A tile [row][16 contraction values], 144-byte pitch
+
 template <int TN>
 struct PDigestSmem {
-    double A[kStages][kKC][kMTP];
+    // orientation 1: A[st][k][row] (kKC x kMTP doubles);  orientation 2: the same bytes as [row][kRowPitch]
+    double A[kStages][(kMT * kRowPitch > kKC * kMTP) ? kMT * kRowPitch : kKC * kMTP];
     double B[kStages][kKC][32 * TN];
     unsigned long long full[kStages];
     unsigned long long empty[kStages];
@@ -122,15 +125,17 @@ __global__ void __launch_bounds__(kDigestThreads, 1) pdigest_kernel(const PDiges
                                     int bytes = (nrows_t - 2 * pc) * 8;
                                     bytes = (c < lc) ? max(0, min(16, bytes)) : 0;
                                     const double* src = bytes ? (Ab + (long long)c * wk.lda + t * kMT + 2 * pc) : g.ring;
-                                    const unsigned sa = (unsigned)__cvta_generic_to_shared(&S.A[st][k][2 * pc]);
+                                    const unsigned sa = (unsigned)__cvta_generic_to_shared(&S.A[st][k * kMTP + 2 * pc]);
                                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(src), "r"(bytes));
                                 }
                             } else {
-#pragma unroll 4
-                                for (int k = 0; k < kKC; ++k) {
-                                    const int c = ch * kKC + k;
-                                    const bool ok = (rowbase >= 0) && (c < lc);
-                                    cp_async8(&S.A[st][k][pt], ok ? (Ab + rowbase + c) : g.ring, ok);
+#pragma unroll
+                                for (int k2i = 0; k2i < kKC / 2; ++k2i) {       // this thread's row: 8 pieces of 16 bytes
+                                    const int c = ch * kKC + 2 * k2i;
+                                    const int bytes = (rowbase >= 0) ? max(0, min(16, (lc - c) * 8)) : 0;
+                                    const double* src = bytes ? (Ab + rowbase + c) : g.ring;
+                                    const unsigned sa = (unsigned)__cvta_generic_to_shared(&S.A[st][pt * kRowPitch + 2 * k2i]);
+                                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(src), "r"(bytes));
                                 }
                             }
                             // B tile: kKC gathered density rows of 32 TN doubles; warp pw copies rows pw, pw+4, ...
@@ -209,10 +214,10 @@ __global__ void __launch_bounds__(kDigestThreads, 1) pdigest_kernel(const PDiges
                 for (int q = 0; q < nch; ++q, ++gch) {
                     const int st = gch % kStages;
                     mbar_wait(&S.full[st], (unsigned)((gch / kStages) & 1));
-                    if (warp_active) {
+                    if (warp_active && wk.orient == 1) {
 #pragma unroll
                         for (int k = 0; k < kKC; ++k) {
-                            const double2* ap = reinterpret_cast<const double2*>(&S.A[st][k][trow]);
+                            const double2* ap = reinterpret_cast<const double2*>(&S.A[st][k * kMTP + trow]);
                             double a[kRows];
 #pragma unroll
                             for (int r = 0; r < kRows / 2; ++r) { const double2 v = ap[r]; a[2 * r] = v.x; a[2 * r + 1] = v.y; }
@@ -231,6 +236,36 @@ __global__ void __launch_bounds__(kDigestThreads, 1) pdigest_kernel(const PDiges
                             for (int r = 0; r < kRows; ++r)
 #pragma unroll
                                 for (int c2 = 0; c2 < kCols; ++c2) acc[r][c2] = fma(a[r], b[c2], acc[r][c2]);
+                        }
+                    } else if (warp_active) {
+                        // orientation 2: row-major tile, two contraction steps per 16-byte operand load
+#pragma unroll
+                        for (int k = 0; k < kKC; k += 2) {
+                            double a0[kRows], a1[kRows];
+#pragma unroll
+                            for (int r = 0; r < kRows; ++r) {
+                                const double2 v = *reinterpret_cast<const double2*>(&S.A[st][(trow + r) * kRowPitch + k]);
+                                a0[r] = v.x; a1[r] = v.y;
+                            }
+#pragma unroll
+                            for (int kk = 0; kk < 2; ++kk) {
+                                double b[kCols];
+                                if constexpr (kWide) {
+#pragma unroll
+                                    for (int c2 = 0; c2 < TN; ++c2) {
+                                        const double2 v = *reinterpret_cast<const double2*>(&S.B[st][k + kk][2 * l16 + 32 * c2]);
+                                        b[2 * c2] = v.x; b[2 * c2 + 1] = v.y;
+                                    }
+                                } else {
+#pragma unroll
+                                    for (int c2 = 0; c2 < TN; ++c2) b[c2] = S.B[st][k + kk][lane + 32 * c2];
+                                }
+#pragma unroll
+                                for (int r = 0; r < kRows; ++r)
+#pragma unroll
+                                    for (int c2 = 0; c2 < kCols; ++c2)
+                                        acc[r][c2] = fma(kk ? a1[r] : a0[r], b[c2], acc[r][c2]);
+                            }
                         }
                     }
                     __syncwarp();
@@ -322,24 +357,37 @@ __global__ void __launch_bounds__(128) pzero_kernel(const PZeroArgs g)
         const PWork wk = g.work[wi];
         const double* __restrict__ qc = (wk.kind ? g.jq : g.pl_q) + wk.clist;
         const double* __restrict__ qr = (wk.kind ? g.jq : g.pl_q) + wk.rlist;
-        for (int m = threadIdx.x; m < wk.nrows; m += blockDim.x) {
-            const int lc = g.tiles[wk.tile0 + m / kDigestRows];
-            const int rdiv = wk.kind ? 1 : (wk.orient == 1 ? wk.nX : wk.nY);
-            const double qrow = qr[m / rdiv];
-            int lo = 0, hi = lc;                                  // first contraction index with Q * Q_row < tau
-            while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] * qrow >= g.tau) lo = mid + 1; else hi = mid; }
+        for (int m0 = 0; m0 < wk.nrows; m0 += blockDim.x) {          // blockDim.x == kDigestRows: one row tile per pass
+            const int m = m0 + threadIdx.x;
+            const bool live = m < wk.nrows;
+            const int lc = g.tiles[wk.tile0 + m0 / kDigestRows];
+            int lo = lc;
+            if (live) {
+                const int rdiv = wk.kind ? 1 : (wk.orient == 1 ? wk.nX : wk.nY);
+                const double qrow = qr[m / rdiv];
+                int a = 0, hi = lc;                               // first contraction index with Q * Q_row < tau
+                while (a < hi) { const int mid = (a + hi) >> 1; if (qc[mid] * qrow >= g.tau) a = mid + 1; else hi = mid; }
+                lo = a;
+            }
             if (wk.orient == 1) {
+                // rows are contiguous in storage: the lanes of a warp walk the contraction index together, so that
+                // the stores of one step are adjacent (rows of a warp have nearly the same cut-off: Q-sorted lists)
+                int lomin = lo;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) lomin = min(lomin, __shfl_xor_sync(0xffffffffu, lomin, o));
                 for (int iy = 0; iy < wk.nY; ++iy) {
                     double* __restrict__ A = g.ring + wk.off + (long long)iy * wk.Lc * wk.lda + m;
-                    for (int cidx = lo; cidx < lc; ++cidx) A[(long long)cidx * wk.lda] = 0.0;
+                    for (int cidx = lomin; cidx < lc; ++cidx)
+                        if (cidx >= lo) A[(long long)cidx * wk.lda] = 0.0;
                 }
-            } else if (wk.kind) {
-                double* __restrict__ A = g.ring + wk.off + (long long)m * wk.lda;
-                for (int cidx = lo; cidx < lc; ++cidx) A[cidx] = 0.0;
-            } else {
-                double* __restrict__ A = g.ring + wk.off + ((long long)(m % wk.nY) * wk.Lc + m / wk.nY) * wk.lda;
-                for (int cidx = lo; cidx < lc; ++cidx)
-                    for (int ix = 0; ix < wk.nX; ++ix) A[(long long)cidx * wk.nX + ix] = 0.0;
+            } else if (live) {
+                if (wk.kind) {
+                    double* __restrict__ A = g.ring + wk.off + (long long)m * wk.lda;
+                    for (int cidx = lo; cidx < lc; ++cidx) A[cidx] = 0.0;
+                } else {
+                    double* __restrict__ A = g.ring + wk.off + ((long long)(m % wk.nY) * wk.Lc + m / wk.nY) * wk.lda;
+                    for (int cidx = lo * wk.nX; cidx < lc * wk.nX; ++cidx) A[cidx] = 0.0;
+                }
             }
         }
     }
@@ -352,7 +400,7 @@ int launch_pzero(ltjk_ctx* c, const PChunk& ch)
     PZeroArgs g;
     g.work = c->d_pwork + ch.work0; g.tiles = c->d_ptile; g.pl_q = c->pl.pl_q; g.jq = c->d_jq;
     g.ring = c->d_pring + (size_t)ch.buf * c->pring_half; g.tau = c->tau; g.nwork = nwork;
-    pzero_kernel<<<std::min(nwork, 148 * 16), 128, 0, c->eri_stream>>>(g);
+    pzero_kernel<<<std::min(nwork, 148 * 16), kDigestRows, 0, c->eri_stream>>>(g);
     LTJK_CUDA(c, cudaGetLastError());
     c->st_launches++;
     return LTJK_OK;
