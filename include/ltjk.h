@@ -93,6 +93,23 @@ int ltjk_build_pseudo_densities(ltjk_ctx* ctx, int nocc, int nvir, const double*
                                 const double* eps_occ, const double* eps_vir, int nT, const double* T,
                                 int ntau, const double* tau_host, double* D_out);
 
+/* No-allocation variant of ltjk_build_pseudo_densities (same operation, same arguments, same result: PAPER.md:L136
+ * Eq. 13, L145 Eq. 15) for callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it.  It calls no cudaMalloc / cudaFree / pool or library allocation and copies nothing from
+ * the host (tau_host is passed to the kernel by value); it only launches three kernels on the ctx stream.  Its
+ * scratch (exponential factors and the half-transformed W) is one static device array of 8 MiB that every GPU which
+ * loads the library holds until the process exits.
+ * Limits (LTJK_EINVAL with a message naming the limit, nothing launched):  ntau <= 32  and
+ *     roundup32(ntau (nocc + nvir)) + ntau nT nocc N  <=  1048576 doubles     (N = number of AOs)
+ * e.g. 160 AO / 20 occupied / 8 points / 4 amplitude sets fits; 439 AO / 81 / 10 / 16 does not (use the plain call).
+ * The array is shared by ALL calls on a device (all contexts, all streams) and keeps the last call's contents; a call
+ * writes every element before reading it, so nothing needs clearing, but two calls that overlap on the GPU race:
+ * serialise them (one stream, or events).  The device address of the array is resolved once per device at
+ * ltjk_create (cudaGetSymbolAddress); if that failed the call returns LTJK_ECUDA. */
+int ltjk_build_pseudo_densities_noalloc(ltjk_ctx* ctx, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                                        const double* eps_occ, const double* eps_vir, int nT, const double* T,
+                                        int ntau, const double* tau_host, double* D_out);
+
 /* Non-symmetric J/K build (steps a5-a9; Eq. 17):
  *   J[d][mu][nu] = sum_{kappa rho} (mu nu|kappa rho) D[d][kappa][rho]
  *   K[d][mu][nu] = sum_{kappa rho} (mu kappa|nu rho) D[d][kappa][rho]

@@ -240,6 +240,7 @@ int ltjk_create(ltjk_ctx** out, int device, void* cuda_stream)
         delete c;
         return LTJK_ECUDA;
     }
+    noalloc_setup(c);      // set-up only: a failure is kept in the context and reported by the no-allocation entry point
     *out = c;
     return LTJK_OK;
 }

@@ -183,6 +183,8 @@ struct ltjk_ctx {
     long long pring_half = 0;              // doubles per half
     int* d_pcounter = nullptr;             // work-stealing cursors, one per digestion launch of a build
     int pcounter_next = 0, pcounter_cap = 0;
+    double* na_scratch = nullptr;          // device address of the static no-allocation scratch (ltjk_transform.cu), per device
+    std::string na_err;                    // why it could not be resolved (reported by the no-allocation entry point)
     bool resident_req = false;             // keep all integral panels of the geometry in HBM across builds (strategy 1)
     bool resident = false, panels_valid = false;
     int digest_mode_req = 0;               // requested: 0 = auto, 1 = block panels (dense), 2 = pair lists
@@ -246,6 +248,7 @@ int launch_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C_occ
                             const double* eps_occ, const double* eps_vir, int nT, const double* T, int ntau,
                             const double* tau_host, double* D_out);
 
+int noalloc_setup(ltjk_ctx* c);            // resolves the static scratch of the no-allocation entry point (set-up)
 int launch_laplace_fock(ltjk_ctx* c, int nD, const double* J, const double* K, int nmo, const double* C, double* F);
 int launch_mo_transform(ltjk_ctx* c, int nD, const double* A, double ca, const double* A2, double ca2, int nmo,
                         const double* C, double* F);

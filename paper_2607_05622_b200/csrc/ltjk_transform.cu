@@ -7,6 +7,8 @@
 #include "ltjk_internal.h"
 #include <algorithm>
 #include <cmath>
+#include <mutex>
+#include <string>
 
 namespace ltjk {
 
@@ -236,4 +238,107 @@ int launch_laplace_accumulate(ltjk_ctx* c, int ntau, int nT, long long nelem, co
     return LTJK_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// No-allocation variant of the pseudo-density transform (include/ltjk.h: ltjk_build_pseudo_densities_noalloc) for
+// callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it).
+// launch_pseudo_densities takes its scratch (exponential factors fo, fv and the half-transformed W) from the
+// stream-ordered pool; here the same scratch lives in ONE file-scope device array of fixed size.  Every GPU that loads
+// the library holds these 8 MiB until the process exits.  All calls (all contexts, all streams) on a device share
+// the array and it keeps the last call's contents: every element a call reads (fo, fv, all of W) is first written by
+// that call's own kernels, so nothing has to start at zero and nothing is cleared; calls that overlap on the GPU race.
+constexpr long long kNoAllocDoubles = 1ll << 20;        // 8 MiB
+constexpr int kNoAllocMaxTau = 32;                      // Laplace points passed by value (the library's grids have <= 14)
+static __device__ __align__(256) double g_noalloc_scratch[kNoAllocDoubles];
+
+struct TauArgs { double tau[kNoAllocMaxTau]; };
+
+// exp_factors_kernel with the Laplace points as kernel arguments: no host-to-device copy, no tau buffer
+__global__ void exp_factors_noalloc_kernel(int nocc, int nvir, int ntau, const double* __restrict__ eo,
+                                           const double* __restrict__ ev, const TauArgs ta,
+                                           double* __restrict__ fo, double* __restrict__ fv)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int n = nocc + nvir;
+    if (t >= ntau * n) return;
+    const int a = t / n, i = t % n;
+    if (i < nocc) fo[a * nocc + i] = exp(eo[i] * ta.tau[a]);
+    else fv[a * nvir + (i - nocc)] = exp(-ev[i - nocc] * ta.tau[a]);
+}
+
+// Set-up, once per device and process (called by ltjk_create with the context's device current).  In host code the
+// NAME g_noalloc_scratch is a host-side stand-in, not a device address: the address the kernels need comes from
+// cudaGetSymbolAddress, per device.
+int noalloc_setup(ltjk_ctx* c)
+{
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static double* ptr_of[kMaxDev] = {};
+    std::lock_guard<std::mutex> lock(mu);
+    c->na_scratch = nullptr;
+    if (c->device < 0 || c->device >= kMaxDev) { c->na_err = "no-allocation scratch: device index beyond 63"; return LTJK_ECUDA; }
+    if (!ptr_of[c->device]) {
+        cudaError_t e = cudaSetDevice(c->device);
+        double* p = nullptr;
+        if (e == cudaSuccess) e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+        if (e != cudaSuccess || !p) {
+            c->na_err = std::string("cudaGetSymbolAddress(g_noalloc_scratch): ") + cudaGetErrorString(e);
+            return LTJK_ECUDA;
+        }
+        ptr_of[c->device] = p;
+    }
+    c->na_scratch = ptr_of[c->device];
+    return LTJK_OK;
+}
+
 }  // namespace ltjk
+
+extern "C" int ltjk_build_pseudo_densities_noalloc(ltjk_ctx* c, int nocc, int nvir, const double* C_occ,
+                                                   const double* C_vir, const double* eps_occ, const double* eps_vir,
+                                                   int nT, const double* T, int ntau, const double* tau_host,
+                                                   double* D_out)
+{
+    using namespace ltjk;
+    if (!c) return LTJK_EINVAL;
+    if (!c->have_basis) return set_err(c, LTJK_ENOBASIS, "build_pseudo_densities_noalloc: no basis");
+    if (nocc <= 0 || nvir <= 0 || nT <= 0 || ntau <= 0 || !C_occ || !C_vir || !eps_occ || !eps_vir || !T || !tau_host ||
+        !D_out)
+        return set_err(c, LTJK_EINVAL, "build_pseudo_densities_noalloc: bad arguments");
+    if (ntau > kNoAllocMaxTau)
+        return set_err(c, LTJK_EINVAL, "build_pseudo_densities_noalloc: ntau = " + std::to_string(ntau) +
+                                           " exceeds the maximum of " + std::to_string(kNoAllocMaxTau) + " Laplace points");
+    const long long N = c->nao;
+    const long long nfac = ((long long)ntau * (nocc + nvir) + 31) & ~31ll;          // W starts 256-byte aligned
+    const long long need = nfac + (long long)ntau * nT * nocc * N;
+    if (need > kNoAllocDoubles)
+        return set_err(c, LTJK_EINVAL, "build_pseudo_densities_noalloc: needs " + std::to_string(need) +
+                                           " doubles of scratch (ntau (nocc + nvir) + ntau nT nocc N), the fixed scratch holds " +
+                                           std::to_string(kNoAllocDoubles) + " (8 MiB); use ltjk_build_pseudo_densities");
+    if (!c->na_scratch) return set_err(c, LTJK_ECUDA, "build_pseudo_densities_noalloc: " + c->na_err);
+    LTJK_CUDA(c, cudaSetDevice(c->device));
+    double* fo = c->na_scratch;
+    double* fv = fo + (long long)ntau * nocc;
+    double* W = c->na_scratch + nfac;
+    TauArgs ta;
+    for (int a = 0; a < kNoAllocMaxTau; ++a) ta.tau[a] = a < ntau ? tau_host[a] : 0.0;
+    const int ne = ntau * (nocc + nvir);
+    exp_factors_noalloc_kernel<<<(ne + 127) / 128, 128, 0, c->stream>>>(nocc, nvir, ntau, eps_occ, eps_vir, ta, fo, fv);
+    LTJK_CUDA(c, cudaGetLastError());
+    GemmArgs g1;   // W[a][d] = (fo[a] .* T[d] .* fv[a]) . C_vir^T        (every element of W is written)
+    g1.M = nocc; g1.Nn = (int)N; g1.K = nvir;
+    g1.A = T; g1.sAa = 0; g1.sAb = (long long)nocc * nvir;
+    g1.B = C_vir; g1.sBa = 0; g1.sBb = 0;
+    g1.C = W; g1.sCa = (long long)nT * nocc * N; g1.sCb = (long long)nocc * N;
+    g1.sr = fo; g1.ssr = nocc; g1.sc = fv; g1.ssc = nvir; g1.nzb = nT; g1.A2 = nullptr; g1.ca = 1.0; g1.ca2 = 0.0;
+    gemm_kernel<true><<<dim3((unsigned)((N + 63) / 64), (nocc + 63) / 64, ntau * nT), 256, 0, c->stream>>>(g1);
+    LTJK_CUDA(c, cudaGetLastError());
+    GemmArgs g2;   // D[a][d] = C_occ . W[a][d]
+    g2.M = (int)N; g2.Nn = (int)N; g2.K = nocc;
+    g2.A = C_occ; g2.sAa = 0; g2.sAb = 0;
+    g2.B = W; g2.sBa = (long long)nT * nocc * N; g2.sBb = (long long)nocc * N;
+    g2.C = D_out; g2.sCa = (long long)nT * N * N; g2.sCb = N * N;
+    g2.sr = nullptr; g2.ssr = 0; g2.sc = nullptr; g2.ssc = 0; g2.nzb = nT; g2.A2 = nullptr; g2.ca = 1.0; g2.ca2 = 0.0;
+    gemm_kernel<false><<<dim3((unsigned)((N + 63) / 64), (unsigned)((N + 63) / 64), ntau * nT), 256, 0, c->stream>>>(g2);
+    LTJK_CUDA(c, cudaGetLastError());
+    c->st_launches += 3;
+    return LTJK_OK;
+}

@@ -22,7 +22,7 @@ ERRORS = {0: "LTJK_OK", -1: "LTJK_EINVAL", -2: "LTJK_ENOBASIS", -3: "LTJK_ECUDA"
 
 EXPORTS = [
     "ltjk_create", "ltjk_destroy", "ltjk_last_error", "ltjk_set_scratch_bytes", "ltjk_set_basis", "ltjk_get_nao",
-    "ltjk_build_shell_pairs", "ltjk_get_schwarz", "ltjk_laplace_quadrature", "ltjk_build_pseudo_densities",
+    "ltjk_build_shell_pairs", "ltjk_get_schwarz", "ltjk_laplace_quadrature", "ltjk_build_pseudo_densities", "ltjk_build_pseudo_densities_noalloc",
     "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_laplace_fock", "ltjk_laplace_accumulate", "ltjk_pp_ladder", "ltjk_get_stats", "ltjk_set_timing", "ltjk_set_digest_mode", "ltjk_get_digest_mode", "ltjk_set_resident", "ltjk_debug_eri_quartet",
     "ltjk_debug_boys", "ltjk_bench_dfma_peak", "ltjk_bench_copy_peak",
 ]
@@ -155,6 +155,16 @@ class Context:
         tau = np.ascontiguousarray(tau, dtype=np.float64)
         nocc, nvir = C_occ.shape[1], C_vir.shape[1]
         self._chk(self.lib.ltjk_build_pseudo_densities(
+            self._h, ctypes.c_int(nocc), ctypes.c_int(nvir), _devptr(C_occ), _devptr(C_vir), _devptr(eps_occ),
+            _devptr(eps_vir), ctypes.c_int(T.shape[0]), _devptr(T), ctypes.c_int(tau.shape[0]), _d(tau),
+            _devptr(D_out)))
+
+    def build_pseudo_densities_noalloc(self, C_occ, C_vir, eps_occ, eps_vir, T, tau, D_out):
+        """ltjk_build_pseudo_densities_noalloc: same arguments and result as build_pseudo_densities; no device
+        allocation (scratch = an 8 MiB static device array shared by all calls; see include/ltjk.h for the limits)."""
+        tau = np.ascontiguousarray(tau, dtype=np.float64)
+        nocc, nvir = C_occ.shape[1], C_vir.shape[1]
+        self._chk(self.lib.ltjk_build_pseudo_densities_noalloc(
             self._h, ctypes.c_int(nocc), ctypes.c_int(nvir), _devptr(C_occ), _devptr(C_vir), _devptr(eps_occ),
             _devptr(eps_vir), ctypes.c_int(T.shape[0]), _devptr(T), ctypes.c_int(tau.shape[0]), _d(tau),
             _devptr(D_out)))
