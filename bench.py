@@ -185,7 +185,7 @@ def run_reference(args, rank, world):
 
 
 def sweep_report(torch, ltjk, w, local, T_host, steps, warmup, world, barrier, max_over_ranks, want_e2e=True, mode=0,
-                 shard=None):
+                 shard=None, quartet_shard=None):
     """Set up one workload (geometry-frozen part outside the timed region), time `steps` whole sweeps with CUDA events
     on the ctx stream, then the per-phase split (timing mode) and the roofline of the digestion kernel."""
     N, nD = w.nao, w.nD
@@ -200,7 +200,19 @@ def sweep_report(torch, ltjk, w, local, T_host, steps, warmup, world, barrier, m
     Co, Cv, eo, ev, Td = dev(w.C_occ), dev(w.C_vir), dev(w.eps_occ), dev(w.eps_vir), dev(T_host)
     D = torch.empty((w.ntau, w.nT, N, N), dtype=torch.float64, device="cuda")
     Dn = D.view(nD, N, N)
-    if shard is None:
+    if quartet_shard is not None:
+        # ONE sweep split in quartet space: partial J, K on every rank, then one all-reduce (sum)
+        from paper_2607_05622_b200.dist import allreduce_jk
+        ctx.set_quartet_shard(*quartet_shard)
+        J = torch.empty_like(Dn)
+        K = torch.empty_like(Dn)
+
+        def step():
+            ctx.build_pseudo_densities(Co, Cv, eo, ev, Td, tau, D)
+            ctx.jk_build(Dn, J, K)
+            allreduce_jk(J, K)
+        want_e2e = False
+    elif shard is None:
         J = torch.empty_like(Dn)
         K = torch.empty_like(Dn)
 
@@ -306,8 +318,10 @@ def main():
     ap.add_argument("--impl", default="ltjk")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mode", type=int, default=0, help="digestion strategy (ltjk_set_digest_mode): 0 auto, 1 panels, 2 pair lists")
-    ap.add_argument("--shard", choices=["problems", "densities"], default="problems",
-                    help="N > 1: every rank its own sweep (weak scaling, default) or ONE sweep's densities dealt round-robin (strong)")
+    ap.add_argument("--shard", choices=["problems", "densities", "quartets"], default="problems",
+                    help="N > 1: every rank its own sweep (weak scaling, default); ONE sweep's densities dealt round-robin "
+                         "(strong, no collective); or ONE sweep's shell quartets split over the ranks with an NCCL "
+                         "all-reduce of J and K inside the timed step (strong)")
     ap.add_argument("--no-large", action="store_true", help="skip the 730-AO sub-run reported under config.large_730")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
@@ -341,9 +355,10 @@ def main():
     # sweep on its own batch of n_T amplitude sets (same molecule, rank-seeded T); no data-path collective.
     from paper_2607_05622_b200.dist import (density_shard, max_over_ranks, rank_amplitudes, sharded_sweep_builds_per_s,
                                             whole_job_builds_per_s)
-    strong = world > 1 and args.shard == "densities"
+    strong = world > 1 and args.shard in ("densities", "quartets")
     T_host = w.T if strong else rank_amplitudes(w, rank)
-    shard = density_shard(nD, rank, world) if strong else None
+    shard = density_shard(nD, rank, world) if (world > 1 and args.shard == "densities") else None
+    qshard = (rank, world) if (world > 1 and args.shard == "quartets") else None
 
     def barrier():
         if world > 1:
@@ -354,7 +369,7 @@ def main():
     if rank == 0:
         sampler.start()
     rep = sweep_report(torch, ltjk, w, local, T_host, args.steps, args.warmup, world, barrier, max_over_ranks, mode=args.mode,
-                       shard=shard)
+                       shard=shard, quartet_shard=qshard)
     clocks = sampler.stop() if rank == 0 else None
     ms_per_step = rep["ms_per_step"]
     value = sharded_sweep_builds_per_s(nD, ms_per_step) if strong else whole_job_builds_per_s(nD, world, ms_per_step)

@@ -171,6 +171,16 @@ int ltjk_set_timing(ltjk_ctx* ctx, int enable);
  *      mode 1 otherwise.
  * Results are the same sums up to rounding order.  Returns LTJK_EINVAL for other values. */
 int ltjk_set_digest_mode(ltjk_ctx* ctx, int mode);
+/* split ONE build over `world` ranks (one process per GPU) in the space of shell quartets.
+ * The launch units of the geometry (block-panel groups, or pair-list chunks: disjoint sets of unique quartets) are
+ * dealt to the ranks by a cost-balanced rule that is a pure function of the geometry, so every rank derives the same
+ * assignment without communication.  After this call ltjk_jk_build generates and digests only the units of `rank`,
+ * for ALL densities: J and K then hold this rank's PARTIAL sums, and the caller adds the partials of all ranks --
+ * one all-reduce (sum) of 2 nD N^2 doubles, e.g. ncclAllReduce through torch.distributed
+ * (paper_2607_05622_b200/dist.py: allreduce_jk).  Every rank holds all of D.  rank = 0, world = 1 (default) is the
+ * whole build.  LTJK_EINVAL unless 0 <= rank < world. */
+int ltjk_set_quartet_shard(ltjk_ctx* ctx, int rank, int world);
+
 /* Geometry-frozen integral cache ("geometry-frozen caches for per-step reuse"), read by the NEXT
  * ltjk_build_shell_pairs; strategy 1 only.  enable != 0: if all canonical integral panels of the geometry fit in
  * 60 % of the free device memory (439 AO: 41 GB) they are generated by the first ltjk_jk_build and kept; later builds

@@ -36,6 +36,24 @@ int ensure_work(ltjk_ctx* c, int nDp)
     return LTJK_OK;
 }
 
+// Owner rank of every launch unit (block-panel group or pair-list chunk) for a split over `world` ranks: longest
+// processing time first onto the least loaded rank.  A pure function of the geometry-frozen work lists, so every rank
+// computes the same assignment without communication; every unit has exactly one owner.
+std::vector<int> unit_owners(const std::vector<double>& cost, int world)
+{
+    std::vector<int> order(cost.size()), owner(cost.size(), 0);
+    for (size_t i = 0; i < cost.size(); ++i) order[i] = (int)i;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cost[a] > cost[b]; });
+    std::vector<double> load(std::max(world, 1), 0.0);
+    for (int i : order) {
+        int best = 0;
+        for (int r = 1; r < world; ++r) if (load[r] < load[best]) best = r;
+        owner[i] = best;
+        load[best] += cost[i];
+    }
+    return owner;
+}
+
 }  // namespace
 
 extern "C" {
@@ -249,8 +267,16 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
         long long gi = 0;
         c->pcounter_next = 0;
         LTJK_CUDA(c, cudaMemsetAsync(c->d_pcounter, 0, sizeof(int) * c->pcounter_cap, c->stream));
+        std::vector<double> cost(c->pchunks.size());
+        for (size_t i = 0; i < cost.size(); ++i)
+            cost[i] = c->pchunks[i].exec_rows_chunks_J + c->pchunks[i].exec_rows_chunks_K + 4.0 * (double)c->pchunks[i].doubles;
+        const std::vector<int> owner = unit_owners(cost, c->shard_world);
+        bool used[2] = {false, false};                // ring half holds a chunk whose digestion may still be running
+        size_t ui = 0;
         for (const PChunk& ch : c->pchunks) {
-            if (!c->timing && gi >= 2) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[ch.buf], 0));
+            if (owner[ui++] != c->shard_rank) continue;                // another rank's share of the quartet space
+            if (!c->timing && used[ch.buf]) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[ch.buf], 0));
+            used[ch.buf] = true;
             if (c->timing) cudaEventRecord(e0, c->stream);
             if ((rc = launch_pzero(c, ch))) return rc;
             if ((rc = launch_peri_chunk(c, ch))) return rc;
@@ -287,8 +313,15 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
         LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_start, 0));
     }
     long long gi = 0;
+    std::vector<double> cost(c->groups.size());
+    for (size_t i = 0; i < cost.size(); ++i) cost[i] = c->groups[i].nints;
+    const std::vector<int> owner = unit_owners(cost, c->shard_world);
+    bool used[2] = {false, false};                    // ring half holds a group whose digestion may still be running
+    size_t ui = 0;
     for (const Group& gr : c->groups) {
-        if (!c->timing && gi >= 2) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[gr.buf], 0));
+        if (owner[ui++] != c->shard_rank) continue;                    // another rank's share of the quartet space
+        if (!c->timing && !c->resident && used[gr.buf]) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[gr.buf], 0));
+        used[gr.buf] = true;
         if (c->timing) cudaEventRecord(e0, c->stream);
         if (!(c->resident && c->panels_valid))
             for (int ck = 0; ck <= gr.cb; ++ck)
@@ -465,6 +498,14 @@ int ltjk_set_digest_mode(ltjk_ctx* c, int mode)
 {
     if (!c || mode < 0 || mode > 2) return LTJK_EINVAL;
     c->digest_mode_req = mode;
+    return LTJK_OK;
+}
+
+int ltjk_set_quartet_shard(ltjk_ctx* c, int rank, int world)
+{
+    if (!c || world < 1 || rank < 0 || rank >= world) return LTJK_EINVAL;
+    if (rank != c->shard_rank || world != c->shard_world) c->panels_valid = false;   // resident panels: other units now
+    c->shard_rank = rank; c->shard_world = world;
     return LTJK_OK;
 }
 

@@ -183,6 +183,7 @@ struct ltjk_ctx {
     long long pring_half = 0;              // doubles per half
     int* d_pcounter = nullptr;             // work-stealing cursors, one per digestion launch of a build
     int pcounter_next = 0, pcounter_cap = 0;
+    int shard_rank = 0, shard_world = 1;   // quartet-space split of one build over ranks (ltjk_set_quartet_shard)
     double* na_scratch = nullptr;          // device address of the static no-allocation scratch (ltjk_transform.cu), per device
     std::string na_err;                    // why it could not be resolved (reported by the no-allocation entry point)
     bool resident_req = false;             // keep all integral panels of the geometry in HBM across builds (strategy 1)

@@ -74,3 +74,18 @@ def gather_sharded(local, n_densities: int):
 def sharded_sweep_builds_per_s(n_densities: int, ms_per_step_max: float) -> float:
     """strong scaling: the job is ONE sweep of n_densities builds split over the ranks"""
     return n_densities / (ms_per_step_max * 1e-3)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Sharding one build in the space of shell quartets (SURVEY.md 8(e), first alternative; 8(f) N5): every rank calls
+# ctx.set_quartet_shard(rank, world), builds its partial J, K for ALL densities, and the partials are summed by ONE
+# all-reduce of 2 nD N^2 doubles (NCCL over NVLink/NVSwitch on GPUs; gloo in the CPU test).  This is the path's only
+# data-plane collective.
+def allreduce_jk(J, K=None):
+    """In-place SUM over ranks of the partial results (torch tensors on the backend's device)."""
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return
+    dist.all_reduce(J, op=dist.ReduceOp.SUM)
+    if K is not None:
+        dist.all_reduce(K, op=dist.ReduceOp.SUM)

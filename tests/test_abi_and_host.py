@@ -100,6 +100,13 @@ for nD in (1, 7, 8, 160):
     full = gather_sharded(fake, nD)
     assert full.shape == (nD, 3, 3) and bool((full[:, 0, 0] == torch.arange(nD, dtype=torch.float64)).all())
 assert abs(sharded_sweep_builds_per_s(160, 500.0) - 320.0) < 1e-12
+# quartet-space split (N5): partial J, K of the ranks are summed in place by one all-reduce
+from paper_2607_05622_b200.dist import allreduce_jk
+Jp = torch.full((2, 4, 4), float(rank + 1), dtype=torch.float64)
+Kp = torch.arange(32, dtype=torch.float64).reshape(2, 4, 4) * (rank + 1)
+allreduce_jk(Jp, Kp)
+tot = world * (world + 1) / 2
+assert bool((Jp == tot).all()) and bool((Kp == torch.arange(32, dtype=torch.float64).reshape(2, 4, 4) * tot).all())
 if rank == 0:
     print("GLOO_OK", v)
 dist.destroy_process_group()

@@ -504,3 +504,30 @@ def test_resident_panels_reused_across_builds(torch_cuda, small):
     J3, K3 = gpu_jk(torch, ctx, D[:8])
     assert ctx.get_stats()["n_launches"] == n_first
     assert relerr(K3[[0, 7]], Kr[:2]) < TOL
+
+
+@pytest.mark.parametrize("mode,scratch,world", [(1, 1 << 20, 2), (1, 1 << 20, 3), (2, 1 << 22, 2), (2, 1 << 22, 5)])
+def test_quartet_shard_partials_sum_to_whole_build(torch_cuda, small, mode, scratch, world):
+    """SURVEY 8(e) / N5 on one GPU: the partial builds of ranks 0..world-1 (ltjk_set_quartet_shard; run one after the
+    other on this device, none waits for another) add up to the whole build, which matches the oracle; no rank's share
+    is empty.  The small scratch gives many launch units to deal out (both digestion strategies)."""
+    torch = torch_cuda
+    w = small
+    D = random_densities(w.nao, 5, seed=61)
+    Jr, Kr, _ = O.jk_folded(w.basis, D, w.schwarz_tau)
+    ctx = make_ctx(w.basis, scratch=scratch, mode=mode)
+    Jsum = np.zeros_like(D)
+    Ksum = np.zeros_like(D)
+    for r in range(world):
+        ctx.set_quartet_shard(r, world)
+        Jp, Kp = gpu_jk(torch, ctx, D)
+        assert np.abs(Kp).max() > 0 and np.abs(Kp).max() < np.abs(Kr).max() * 1.5
+        Jsum += Jp
+        Ksum += Kp
+    assert relerr(Jsum, Jr) < TOL and relerr(Ksum, Kr) < TOL
+    ctx.set_quartet_shard(0, 1)
+    J, K = gpu_jk(torch, ctx, D)
+    assert relerr(Jsum, J) < 1e-12 and relerr(Ksum, K) < 1e-12
+    from paper_2607_05622_b200 import ltjk
+    with pytest.raises(ltjk.LtjkError):
+        ctx.set_quartet_shard(2, 2)
