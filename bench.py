@@ -401,8 +401,14 @@ def main():
     single_point = {"n_D": int(w.nT), "ms": e0.elapsed_time(e1), "builds_per_s": w.nT / (e0.elapsed_time(e1) * 1e-3)}
     measured = json.loads((ROOT / "MEASURED_PEAKS.json").read_text()) if (ROOT / "MEASURED_PEAKS.json").exists() else {}
     hbm_peak = measured.get("hbm_gbs", hbm_gbs)
+    # the transform is a dense fp64 contraction (DMMA): its roof is the fp64 tensor peak, taken as the measured bf16
+    # tensor peak x the guide's nominal ratio 45 / 2250 (blackwell_cuda_programming.md: B200 FP64 tensor 45 TFLOP/s);
+    # at that roof it would write D at ~0.9 TB/s, so the HBM fraction asked for by north_star cannot exceed ~0.14
+    f64_tensor_peak = measured.get("bf16_tflops", 1605.6) * 45.0 / 2250.0
     transform = dict(rep["transform"], frac_of_hbm_peak=rep["transform"]["gbs_written"] / hbm_peak, hbm_peak_gbs=hbm_peak,
-                     hbm_peak_source="MEASURED_PEAKS.json" if "hbm_gbs" in measured else "copy microbenchmark in this run")
+                     hbm_peak_source="MEASURED_PEAKS.json" if "hbm_gbs" in measured else "copy microbenchmark in this run",
+                     bound="tensor (f64 DMMA)", f64_tensor_peak_tflops=f64_tensor_peak,
+                     frac_of_f64_tensor_peak=rep["transform"]["tflops"] / f64_tensor_peak)
     cpu = None
     if not args.no_cpu_baseline:
         cpu = oracle_sample(w, Dn.cpu().numpy(), target_s=20.0)
