@@ -24,10 +24,14 @@
  *                          in oracle/oracle.py)
  *   orc_schwarz        O8  Q_AB = sqrt(max |(ab|ab)|)
  *   orc_jk_blocks          J and K blocks for sampled shell pairs straight from Eq. (17) (full-size sampling)
+ *   orc_jk_grad            SURVEY 8(f) N2: derivative builds J^x(A,B), K^x(A,B), Eq. (18), written out
+ *                          term by term (one term per differentiated function), no symmetry used
  *
  * Pins (tests/test_oracle_*.py): Boys vs mpmath quadrature / gammainc / closed forms; (ss|ss) closed form,
  * 2 sqrt(a/pi), erf(sqrt(rho) R)/R; finite differences in the centre for p and d; 8-fold symmetry of O7;
- * Cauchy-Schwarz, PSD; translation/rotation invariance; O6 vs O7; J/K symmetry relations.
+ * Cauchy-Schwarz, PSD; translation/rotation invariance; O6 vs O7; J/K symmetry relations; orc_jk_grad: central finite
+ * differences of tr(A^T J[B]), tr(A^T K[B]) built from orc_eri_tensor, closed form d/dR [erf(sqrt(rho) R)/R], the
+ * translational sum rule Eq. (31), J^x(A,B) = J^x(B,A), K^x(A,B) = K^x(B,A) = K^x(A^T,B^T)  (tests/test_oracle_grad.py).
  * Nothing here is "parity unpinned".
  */
 #include <math.h>
@@ -35,10 +39,12 @@
 #include <string.h>
 #include <omp.h>
 
-#define LMAXSH 2
-#define LTOT (4 * LMAXSH)          /* 8 */
-#define NH1 (2 * LMAXSH + 1)       /* Hermite orders per pair and dimension: 0..4 */
-#define NR (LTOT + 1)              /* 9 */
+#define LMAXSH 2                   /* largest angular momentum of an input shell */
+#define LMAXW 3                    /* largest angular momentum inside eri_shell: the derivative builds (orc_jk_grad) raise ONE index by one */
+#define LTOT (3 * LMAXSH + LMAXW)  /* 9 */
+#define NH1 (2 * LMAXW + 1)        /* Hermite orders per pair and dimension */
+#define NR (LTOT + 1)              /* 10 */
+#define NCMAX 10                   /* Cartesian components of an l = LMAXW shell */
 
 static const double PI = 3.14159265358979323846264338327950288;
 
@@ -82,11 +88,11 @@ void orc_boys(int mmax, double T, double *F)
  *   E_t^{i+1,j} = E_{t-1}^{ij}/(2p) + X_PA E_t^{ij} + (t+1) E_{t+1}^{ij}
  *   E_t^{i,j+1} = E_{t-1}^{ij}/(2p) + X_PB E_t^{ij} + (t+1) E_{t+1}^{ij}           (zero outside 0<=t<=i+j) */
 static void hermite_E(int la, int lb, double a, double b, double XA, double XB,
-                      double E[LMAXSH + 1][LMAXSH + 1][NH1])
+                      double E[LMAXW + 1][LMAXW + 1][NH1])
 {
     double p = a + b, mu = a * b / p, XAB = XA - XB, XP = (a * XA + b * XB) / p;
     double XPA = XP - XA, XPB = XP - XB;
-    memset(E, 0, sizeof(double) * (LMAXSH + 1) * (LMAXSH + 1) * NH1);
+    memset(E, 0, sizeof(double) * (LMAXW + 1) * (LMAXW + 1) * NH1);
     E[0][0][0] = exp(-mu * XAB * XAB);
     for (int i = 0; i <= la; ++i) {
         if (i > 0)   /* raise i: from (i-1, 0) */
@@ -154,7 +160,7 @@ static void eri_shell(const basis_t *bs, int A, int B, int C, int D, double *out
     int la = bs->l[A], lb = bs->l[B], lc = bs->l[C], ld = bs->l[D];
     int na = ncart(la), nb = ncart(lb), nc = ncart(lc), nd = ncart(ld);
     int L = la + lb + lc + ld;
-    int ca[6][3], cb[6][3], cc[6][3], cd[6][3];
+    int ca[NCMAX][3], cb[NCMAX][3], cc[NCMAX][3], cd[NCMAX][3];
     cart_list(la, ca); cart_list(lb, cb); cart_list(lc, cc); cart_list(ld, cd);
     const double *RA = bs->xyz + 3 * bs->atom[A], *RB = bs->xyz + 3 * bs->atom[B];
     const double *RC = bs->xyz + 3 * bs->atom[C], *RD = bs->xyz + 3 * bs->atom[D];
@@ -166,7 +172,7 @@ static void eri_shell(const basis_t *bs, int A, int B, int C, int D, double *out
         double a = bs->exps[bs->prim_off[A] + ia], b = bs->exps[bs->prim_off[B] + ib];
         double cab = bs->coef[bs->prim_off[A] + ia] * bs->coef[bs->prim_off[B] + ib];
         double p = a + b, P[3];
-        double Eab[3][LMAXSH + 1][LMAXSH + 1][NH1];
+        double Eab[3][LMAXW + 1][LMAXW + 1][NH1];
         for (int x = 0; x < 3; ++x) {
             P[x] = (a * RA[x] + b * RB[x]) / p;
             hermite_E(la, lb, a, b, RA[x], RB[x], Eab[x]);
@@ -176,7 +182,7 @@ static void eri_shell(const basis_t *bs, int A, int B, int C, int D, double *out
             double c = bs->exps[bs->prim_off[C] + ic], d = bs->exps[bs->prim_off[D] + id];
             double ccd = bs->coef[bs->prim_off[C] + ic] * bs->coef[bs->prim_off[D] + id];
             double q = c + d, Q[3], PQ[3];
-            double Ecd[3][LMAXSH + 1][LMAXSH + 1][NH1];
+            double Ecd[3][LMAXW + 1][LMAXW + 1][NH1];
             for (int x = 0; x < 3; ++x) {
                 Q[x] = (c * RC[x] + d * RD[x]) / q;
                 PQ[x] = P[x] - Q[x];
@@ -431,6 +437,101 @@ void orc_jk_blocks(BASIS_ARGS, double tau, int nD, const double *D, int nblk, co
         }
     }
     free(Q); free(off);
+}
+
+/* SURVEY 8(f) N2.  Derivative (skeleton) builds, Eq. (18), with the nuclear derivative written out by the
+ * product rule, one term per function of the integral (Eqs. (30)-(31): the centre derivatives):
+ *   J^x(A,B) = sum_{mnkr} (mn|kr)^x A_mn B_kr ,   K^x(A,B) = sum_{mnkr} (mk|nr)^x A_mn B_kr ,
+ *   (mn|kr)^x = (d_x m n|kr) + (m d_x n|kr) + (mn|d_x k r) + (mn|k d_x r) ,  d_x = derivative with respect to coordinate
+ *   x of the atom that carries the function (zero for the other atoms).
+ * A Cartesian Gaussian differentiates into one function of l+1 and one of l-1 on the same centre, primitive by primitive:
+ *   d/dA_x [ x_A^i y_A^j z_A^k sum_p c_p e^{-a_p r_A^2} ] = x_A^{i+1} y_A^j z_A^k sum_p (2 a_p c_p) e^{-a_p r_A^2}
+ *                                                          - i x_A^{i-1} y_A^j z_A^k sum_p c_p e^{-a_p r_A^2} ,
+ * so every term is an ordinary integral (O5) over an auxiliary shell list: shell s raised (l+1, coefficients 2 a_p c_p)
+ * and shell s lowered (l-1, coefficients c_p).  Every ORDERED shell quartet and every position is evaluated on its
+ * own; no permutational symmetry, no screening, no prefactors.
+ * A, B: [nP][N][N] row-major (general, non-symmetric).  gJ, gK: [nP][natom][3], overwritten. */
+static int cart_index(int l, int i, int j, int k)
+{
+    int c[NCMAX][3];
+    cart_list(l, c);
+    for (int n = 0; n < ncart(l); ++n) if (c[n][0] == i && c[n][1] == j && c[n][2] == k) return n;
+    return -1;
+}
+
+void orc_jk_grad(BASIS_ARGS, int nP, const double *A, const double *B, double *gJ, double *gK)
+{
+    basis_t bs = BASIS_INIT;
+    int ns = nshell, ntotp = 0;
+    for (int s = 0; s < ns; ++s) if (prim_off[s] + nprim[s] > ntotp) ntotp = prim_off[s] + nprim[s];
+    /* auxiliary shell list: [0,ns) the shells, [ns,2ns) raised, [2ns,3ns) lowered */
+    int *xa = (int *)malloc(sizeof(int) * 3 * ns), *xl = (int *)malloc(sizeof(int) * 3 * ns);
+    int *xn = (int *)malloc(sizeof(int) * 3 * ns), *xo = (int *)malloc(sizeof(int) * 3 * ns);
+    double *xe = (double *)malloc(sizeof(double) * 3 * ntotp), *xc = (double *)malloc(sizeof(double) * 3 * ntotp);
+    for (int v = 0; v < 3; ++v) {
+        for (int i = 0; i < ntotp; ++i) {
+            xe[v * ntotp + i] = exps[i];
+            xc[v * ntotp + i] = (v == 1) ? 2.0 * exps[i] * coef[i] : coef[i];
+        }
+        for (int s = 0; s < ns; ++s) {
+            xa[v * ns + s] = atom[s]; xn[v * ns + s] = nprim[s]; xo[v * ns + s] = v * ntotp + prim_off[s];
+            xl[v * ns + s] = (v == 0) ? l[s] : (v == 1) ? l[s] + 1 : (l[s] > 0 ? l[s] - 1 : 0);
+        }
+    }
+    basis_t aux = { natom, xyz, 3 * ns, xa, xl, xn, xo, xe, xc };
+    int *off = (int *)malloc(sizeof(int) * (ns + 1));
+    ao_offsets(&bs, off);
+    long N = off[ns];
+    long ng = (long)nP * natom * 3;
+    for (long i = 0; i < ng; ++i) gJ[i] = gK[i] = 0.0;
+#pragma omp parallel
+    {
+        double *up = (double *)malloc(sizeof(double) * NCMAX * 216), *dn = (double *)malloc(sizeof(double) * NCMAX * 216);
+        double *lj = (double *)calloc((size_t)ng, sizeof(double)), *lk = (double *)calloc((size_t)ng, sizeof(double));
+#pragma omp for collapse(2) schedule(dynamic)
+        for (int M = 0; M < ns; ++M)
+        for (int Nn = 0; Nn < ns; ++Nn)
+            for (int K = 0; K < ns; ++K)
+            for (int R = 0; R < ns; ++R) {
+                const int sh[4] = { M, Nn, K, R };
+                int nc[4], cl[4][NCMAX][3];
+                for (int q = 0; q < 4; ++q) { nc[q] = ncart(l[sh[q]]); cart_list(l[sh[q]], cl[q]); }
+                for (int pos = 0; pos < 4; ++pos) {
+                    const int S = sh[pos], ls = l[S], at = atom[S];
+                    int su[4] = { M, Nn, K, R }, sd[4] = { M, Nn, K, R };
+                    su[pos] = ns + S; sd[pos] = 2 * ns + S;
+                    int nu[4] = { nc[0], nc[1], nc[2], nc[3] }, nd[4] = { nc[0], nc[1], nc[2], nc[3] };
+                    nu[pos] = ncart(ls + 1); nd[pos] = ls > 0 ? ncart(ls - 1) : 1;
+                    eri_shell(&aux, su[0], su[1], su[2], su[3], up);
+                    if (ls > 0) eri_shell(&aux, sd[0], sd[1], sd[2], sd[3], dn);
+                    int c[4];
+                    for (c[0] = 0; c[0] < nc[0]; ++c[0]) for (c[1] = 0; c[1] < nc[1]; ++c[1])
+                    for (c[2] = 0; c[2] < nc[2]; ++c[2]) for (c[3] = 0; c[3] < nc[3]; ++c[3]) {
+                        const long m = off[M] + c[0], n = off[Nn] + c[1], k = off[K] + c[2], r = off[R] + c[3];
+                        for (int x = 0; x < 3; ++x) {
+                            int e[3] = { cl[pos][c[pos]][0], cl[pos][c[pos]][1], cl[pos][c[pos]][2] };
+                            int cu[4] = { c[0], c[1], c[2], c[3] }, cd_[4] = { c[0], c[1], c[2], c[3] };
+                            e[x] += 1; cu[pos] = cart_index(ls + 1, e[0], e[1], e[2]); e[x] -= 1;
+                            double dI = up[((cu[0] * nu[1] + cu[1]) * nu[2] + cu[2]) * nu[3] + cu[3]];
+                            if (e[x] > 0) {
+                                const int pw = e[x];
+                                e[x] -= 1; cd_[pos] = cart_index(ls - 1, e[0], e[1], e[2]); e[x] += 1;
+                                dI -= pw * dn[((cd_[0] * nd[1] + cd_[1]) * nd[2] + cd_[2]) * nd[3] + cd_[3]];
+                            }
+                            for (int p = 0; p < nP; ++p) {
+                                const double *Ap = A + (size_t)p * N * N, *Bp = B + (size_t)p * N * N;
+                                lj[((long)p * natom + at) * 3 + x] += dI * Ap[m * N + n] * Bp[k * N + r];   /* (mn|kr)^x A_mn B_kr */
+                                lk[((long)p * natom + at) * 3 + x] += dI * Ap[m * N + k] * Bp[n * N + r];   /* (mn|kr)^x A_mk B_nr */
+                            }
+                        }
+                    }
+                }
+            }
+#pragma omp critical
+        for (long i = 0; i < ng; ++i) { gJ[i] += lj[i]; gK[i] += lk[i]; }
+        free(up); free(dn); free(lj); free(lk);
+    }
+    free(xa); free(xl); free(xn); free(xo); free(xe); free(xc); free(off);
 }
 
 int orc_max_threads(void) { return omp_get_max_threads(); }

@@ -156,6 +156,20 @@ def jk_blocks(b, D: np.ndarray, tau: float, shell_pairs, Q=None):
     return Js, Ks
 
 
+def jk_grad(b, A: np.ndarray, B: np.ndarray):
+    """J^x(A,B), K^x(A,B) of Eq. (18) for nP density pairs; returns two arrays
+    [nP, natom, 3].  Plain product rule over the four functions of every ordered shell quartet (orc_jk_grad)."""
+    args, keep = _basis_args(b)
+    A = np.ascontiguousarray(A, dtype=np.float64)
+    B = np.ascontiguousarray(B, dtype=np.float64)
+    nP = A.shape[0]
+    natom = np.asarray(b.xyz).shape[0]
+    gJ = np.zeros((nP, natom, 3))
+    gK = np.zeros((nP, natom, 3))
+    lib().orc_jk_grad(*args, ctypes.c_int(nP), _d(A), _d(B), _d(gJ), _d(gK))
+    return gJ, gK
+
+
 # ---------------------------------------------------------------------------------------------------------
 # O10 pseudo-density, explicit loops (Eqs. (13), (15)):  D^{alpha,d}_{mu nu} =
 #     sum_{ia} C_{mu i} e^{+eps_i tau_alpha} T^d_{ia} e^{-eps_a tau_alpha} C_{nu a}
