@@ -469,6 +469,27 @@ def main():
         del D1, J1, K1, X, Lo
         c2.close()
         torch.cuda.empty_cache()
+        # N2: derivative builds J^x(A,B), K^x(A,B) (Eq. 18) on the 160-AO workload, 4 non-symmetric density pairs
+        ws = make_workload("small")
+        c3 = ltjk.Context(local, stream)
+        c3.set_basis(ws.basis)
+        Ag = torch.from_numpy(1e-2 * rng.standard_normal((4, ws.nao, ws.nao))).cuda()
+        Bg = torch.from_numpy(1e-2 * rng.standard_normal((4, ws.nao, ws.nao))).cuda()
+        gJ = torch.empty((4, ws.basis.xyz.shape[0], 3), dtype=torch.float64, device="cuda")
+        gK = torch.empty_like(gJ)
+        c3.jk_grad(Ag, Bg, gJ, gK)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        c3.jk_grad(Ag, Bg, gJ, gK)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        nq = ws.basis.nshell ** 2 * (ws.basis.nshell * (ws.basis.nshell + 1) // 2)
+        config["jk_grad"] = {"workload": "small (160 AO, 73 shells, 14 atoms), 4 density pairs, no screening",
+                             "ms": e0.elapsed_time(e1), "shell_quartet_derivatives_per_s": nq / (e0.elapsed_time(e1) * 1e-3),
+                             "note": "J^x(A,B), K^x(A,B) of Eq. 18 (SURVEY 8(f) N2): first correct version, one thread per "
+                                     "(M, N, {K,R}), derivative integrals contracted on the fly"}
+        launches += c3.get_stats()["n_launches"]
+        c3.close()
     if world == 1 and not args.no_large and w.name != "large":
         wl = make_workload("large")
         s2 = ClockSampler(local)

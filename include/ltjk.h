@@ -152,6 +152,17 @@ int ltjk_laplace_accumulate(ltjk_ctx* ctx, int ntau, int nT, long long nelem, co
  * enqueued on the ctx stream; scratch of 2 * chunk * N^2 doubles is taken from the stream-ordered pool. */
 int ltjk_pp_ladder(ltjk_ctx* ctx, int nvir, const double* C_vir, int npair, const double* X, double* L, int chunk);
 
+/* derivative (skeleton) builds, Eq. 18 with the centre derivatives of L382-386
+ * (Eqs. 30-31), for nP ordered pairs of general (non-symmetric) AO densities:
+ *     gradJ[p][at][x] = sum_{mnkr} d(mn|kr)/dX_{at,x} A[p][m][n] B[p][k][r]
+ *     gradK[p][at][x] = sum_{mnkr} d(mk|nr)/dX_{at,x} A[p][m][n] B[p][k][r]        (X = nuclear coordinates, bohr)
+ * bare builds, no prefactors; the derivative acts on every function centred on atom `at`.
+ * A, B: DEVICE [nP][N][N] row-major in the caller's AO order; gradJ, gradK: DEVICE [nP][natom][3], overwritten
+ * (one of them may be NULL).  Needs ltjk_set_basis only.  EVERY shell quartet is evaluated (no Schwarz screening: a
+ * value bound does not bound a derivative), so the cost is O(nshell^4); meant for the sizes of the tiny / small
+ * configs.  Work is enqueued on the ctx stream; the first call after ltjk_set_basis uploads the basis (allocates). */
+int ltjk_jk_grad(ltjk_ctx* ctx, int nP, const double* A, const double* B, double* gradJ, double* gradK);
+
 /* Statistics of the last ltjk_jk_build on this context (HOST outputs, any may be NULL):
  *   n_launches    kernels launched
  *   eri_quartets  contracted shell quartets evaluated (4-fold unique: A>=B, C>=D, all bra x ket)

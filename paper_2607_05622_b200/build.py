@@ -21,7 +21,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 CU_SOURCES = ["ltjk_api.cu", "ltjk_build.cu", "ltjk_eri.cu", "ltjk_digest.cu", "ltjk_transform.cu", "ltjk_pair.cu",
-              "ltjk_peri.cu", "ltjk_pdigest.cu"]
+              "ltjk_peri.cu", "ltjk_pdigest.cu", "ltjk_grad.cu"]
 CPP_SOURCES = ["ltjk_laplace.cpp"]
 HEADERS = ["ltjk_internal.h", "digest_common.h", "eri_core.h", "boys_table.h", "../../include/ltjk.h", "gen_eri.py"]
 
@@ -38,6 +38,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         subprocess.check_call([sys.executable, str(CSRC / "gen_eri.py"), str(GEN)])
     hdr_time = max(_mtime(CSRC / h) for h in HEADERS)
     hdr_time = max(hdr_time, _mtime(gen_h))
+    if not (GEN / "eri_gen_d1.h").exists():
+        subprocess.check_call([sys.executable, str(CSRC / "gen_eri.py"), str(GEN)])
     jobs = []
     for src in CU_SOURCES:
         obj = OBJ / (src + ".o")

@@ -14,6 +14,9 @@
 #endif
 
 #include "gen/eri_gen.h"
+#ifdef LTJK_WITH_D1
+#include "gen/eri_gen_d1.h"     // f-raised classes, only for ltjk_grad.cu
+#endif
 
 namespace ltjk {
 
@@ -24,7 +27,7 @@ constexpr int kPairStride = kPairHeader + kMaxPrimPair * kPrimStride;   // doubl
 
 // Boys table: F_m(T_i), T_i = i/8, i = 0..288 (T <= 36), m = 0..16
 constexpr int kBoysNT = 289;
-constexpr int kBoysNM = 17;
+constexpr int kBoysNM = 18;          // orders 0..17: L <= 9 (derivative builds) plus 8 Taylor terms
 constexpr double kBoysTmax = 36.0;
 constexpr int kBoysTaylor = 9;        // terms k = 0..8: remainder (1/16)^9/9! ~ 4e-17
 

@@ -239,6 +239,54 @@ def main(out_dir):
             hdr.append("};")
     hdr.append("} // namespace ltjk_gen")
     (out / "eri_gen.h").write_text("\n".join(hdr) + "\n")
+    # ---- classes with ONE index raised to l = 3, for the first-derivative builds (ltjk_grad.cu):
+    # d/dA_x of a shell of l is a shell of l + 1 (and one of l - 1), so (f b|c d) with b, c, d <= 2 is all that is needed.
+    d1 = ["// GENERATED by gen_eri.py -- do not edit.  f-raised classes for the derivative builds (see gen_eri.py).",
+          "#pragma once", "namespace ltjk_gen {"]
+    for lb in range(LMAX + 1):
+        body = gen_hrr(LMAX + 1, lb)
+        d1.append("template<> struct Hrr<%d,%d> {" % (LMAX + 1, lb))
+        d1.append("  static constexpr int NE = %d;" % len(range_index(LMAX + 1, LMAX + 1 + lb)))
+        d1.append("  static constexpr int NAB = %d;" % (ncart(LMAX + 1) * ncart(lb)))
+        d1.append("  LTJK_HD static void run(const double* __restrict__ src, const int ss, double* __restrict__ dst, "
+                  "const int ds, const double ABx, const double ABy, const double ABz) {")
+        d1.append("    (void)ABx; (void)ABy; (void)ABz;")
+        for ln in body:
+            d1.append("    " + ln)
+        d1.append("  }")
+        d1.append("};")
+    for lb in range(LMAX + 1):
+        for (lc, ld) in PAIR_CLASSES:
+            g = VRR(LMAX + 1, lb, lc, ld)
+            body, ne, nf = g.generate()
+            stats.append(((LMAX + 1, lb, lc, ld), g.n, ne * nf))
+            d1.append("template<> struct Vrr<%d,%d,%d,%d> {" % (LMAX + 1, lb, lc, ld))
+            d1.append("  static constexpr int NE = %d, NF = %d, NNODE = %d;" % (ne, nf, g.n))
+            d1.append("  template<class SINK> LTJK_HD static void run_t(const double* __restrict__ F, "
+                      "const double PAx, const double PAy, const double PAz, "
+                      "const double WPx, const double WPy, const double WPz, "
+                      "const double QCx, const double QCy, const double QCz, "
+                      "const double WQx, const double WQy, const double WQz, "
+                      "const double oo2p, const double oo2q, const double oo2pq, "
+                      "const double rp, const double rq, SINK& sink) {")
+            d1.append("    (void)PAx;(void)PAy;(void)PAz;(void)WPx;(void)WPy;(void)WPz;(void)QCx;(void)QCy;(void)QCz;"
+                      "(void)WQx;(void)WQy;(void)WQz;(void)oo2p;(void)oo2q;(void)oo2pq;(void)rp;(void)rq;")
+            for ln in body:
+                d1.append("    " + ln)
+            d1.append("  }")
+            d1.append("  LTJK_HD static void run(const double* __restrict__ F, "
+                      "const double PAx, const double PAy, const double PAz, "
+                      "const double WPx, const double WPy, const double WPz, "
+                      "const double QCx, const double QCy, const double QCz, "
+                      "const double WQx, const double WQy, const double WQz, "
+                      "const double oo2p, const double oo2q, const double oo2pq, "
+                      "const double rp, const double rq, double* __restrict__ acc) {")
+            d1.append("    AccSink s{acc};")
+            d1.append("    run_t(F, PAx, PAy, PAz, WPx, WPy, WPz, QCx, QCy, QCz, WQx, WQy, WQz, oo2p, oo2q, oo2pq, rp, rq, s);")
+            d1.append("  }")
+            d1.append("};")
+    d1.append("} // namespace ltjk_gen")
+    (out / "eri_gen_d1.h").write_text("\n".join(d1) + "\n")
     with open(out / "eri_gen_stats.txt", "w") as fh:
         fh.write("# class(la lb lc ld)  vrr_nodes_per_primitive_quartet  contracted_accumulators\n")
         for cls, n, na in stats:

@@ -183,6 +183,9 @@ struct ltjk_ctx {
     long long pring_half = 0;              // doubles per half
     int* d_pcounter = nullptr;             // work-stealing cursors, one per digestion launch of a build
     int pcounter_next = 0, pcounter_cap = 0;
+    double *gr_xyz = nullptr, *gr_exps = nullptr, *gr_coef = nullptr;   // basis in caller order for ltjk_jk_grad (ltjk_grad.cu)
+    int* gr_int = nullptr;
+    int gr_cnt[3] = {0, 0, 0};
     int shard_rank = 0, shard_world = 1;   // quartet-space split of one build over ranks (ltjk_set_quartet_shard)
     double* na_scratch = nullptr;          // device address of the static no-allocation scratch (ltjk_transform.cu), per device
     std::string na_err;                    // why it could not be resolved (reported by the no-allocation entry point)
@@ -248,6 +251,10 @@ int bench_copy(ltjk_ctx* c, double* gbs);
 int launch_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C_occ, const double* C_vir,
                             const double* eps_occ, const double* eps_vir, int nT, const double* T, int ntau,
                             const double* tau_host, double* D_out);
+
+// ltjk_grad.cu
+void free_grad(ltjk_ctx* c);
+int launch_jk_grad(ltjk_ctx* c, int nP, const double* A, const double* B, double* gJ, double* gK);
 
 int noalloc_setup(ltjk_ctx* c);            // resolves the static scratch of the no-allocation entry point (set-up)
 int launch_laplace_fock(ltjk_ctx* c, int nD, const double* J, const double* K, int nmo, const double* C, double* F);

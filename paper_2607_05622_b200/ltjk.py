@@ -23,7 +23,7 @@ ERRORS = {0: "LTJK_OK", -1: "LTJK_EINVAL", -2: "LTJK_ENOBASIS", -3: "LTJK_ECUDA"
 EXPORTS = [
     "ltjk_create", "ltjk_destroy", "ltjk_last_error", "ltjk_set_scratch_bytes", "ltjk_set_basis", "ltjk_get_nao",
     "ltjk_build_shell_pairs", "ltjk_get_schwarz", "ltjk_laplace_quadrature", "ltjk_build_pseudo_densities", "ltjk_build_pseudo_densities_noalloc",
-    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_laplace_fock", "ltjk_laplace_accumulate", "ltjk_pp_ladder", "ltjk_get_stats", "ltjk_set_timing", "ltjk_set_digest_mode", "ltjk_get_digest_mode", "ltjk_set_resident", "ltjk_set_quartet_shard", "ltjk_debug_eri_quartet",
+    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_laplace_fock", "ltjk_laplace_accumulate", "ltjk_pp_ladder", "ltjk_jk_grad", "ltjk_get_stats", "ltjk_set_timing", "ltjk_set_digest_mode", "ltjk_get_digest_mode", "ltjk_set_resident", "ltjk_set_quartet_shard", "ltjk_debug_eri_quartet",
     "ltjk_debug_boys", "ltjk_bench_dfma_peak", "ltjk_bench_copy_peak",
 ]
 
@@ -131,6 +131,7 @@ class Context:
         self._chk(self.lib.ltjk_get_nao(self._h, ctypes.byref(n)))
         self.nao = n.value
         self.nshell = int(l.shape[0])
+        self.natom = int(xyz.shape[0])
 
     def get_nao(self) -> int:
         n = ctypes.c_int(0)
@@ -224,6 +225,11 @@ class Context:
         """ltjk_pp_ladder: L[p] = C_vir^T K[C_vir X[p] C_vir^T] C_vir = sum_ef (ae|bf) X[p,e,f]; device tensors."""
         self._chk(self.lib.ltjk_pp_ladder(self._h, ctypes.c_int(C_vir.shape[1]), _devptr(C_vir),
                                           ctypes.c_int(X.shape[0]), _devptr(X), _devptr(L), ctypes.c_int(int(chunk))))
+
+    def jk_grad(self, A, B, gradJ, gradK):
+        """ltjk_jk_grad: J^x(A,B), K^x(A,B) (Eq. 18) for device tensors A, B [nP,N,N] -> gradJ, gradK [nP,natom,3]."""
+        self._chk(self.lib.ltjk_jk_grad(self._h, ctypes.c_int(A.shape[0]), _devptr(A), _devptr(B), _devptr(gradJ),
+                                        _devptr(gradK)))
 
     def get_stats(self) -> dict:
         nl = ctypes.c_longlong(0)

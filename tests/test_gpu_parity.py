@@ -531,3 +531,57 @@ def test_quartet_shard_partials_sum_to_whole_build(torch_cuda, small, mode, scra
     from paper_2607_05622_b200 import ltjk
     with pytest.raises(ltjk.LtjkError):
         ctx.set_quartet_shard(2, 2)
+
+
+def gpu_grad(torch, ctx, A, B):
+    Ad, Bd = torch.from_numpy(np.ascontiguousarray(A)).cuda(), torch.from_numpy(np.ascontiguousarray(B)).cuda()
+    natom = ctx.natom
+    gJ = torch.full((A.shape[0], natom, 3), float("nan"), dtype=torch.float64, device="cuda")
+    gK = torch.full_like(gJ, float("nan"))
+    ctx.jk_grad(Ad, Bd, gJ, gK)
+    torch.cuda.synchronize()
+    return gJ.cpu().numpy(), gK.cpu().numpy()
+
+
+def test_jk_grad_vs_oracle(torch_cuda, tiny, spd_basis):
+    """SURVEY 8(f) N2 (Eq. 18; L382-386): derivative builds J^x(A,B), K^x(A,B) for pairs of non-symmetric
+    densities against the oracle's term-by-term product rule, element by element.  tiny: s, p (uncontracted);
+    spd: contracted s, p, d on three atoms (every one of the 54 kernel classes, raised f classes included); 6 pairs =
+    two launches of 4 + 2.  Also the translational sum rule (Eq. 31) on the GPU result itself."""
+    from paper_2607_05622_b200 import ltjk
+    torch = torch_cuda
+    for b in (tiny.basis, spd_basis):
+        A = random_densities(b.nao, 6, seed=71)
+        B = random_densities(b.nao, 6, seed=72)
+        ctx = ltjk.Context(0)
+        ctx.set_basis(b)
+        gJ, gK = gpu_grad(torch, ctx, A, B)
+        rJ, rK = O.jk_grad(b, A, B)
+        assert np.abs(gJ - rJ).max() <= TOL * np.abs(rJ).max(), np.abs(gJ - rJ).max() / np.abs(rJ).max()
+        assert np.abs(gK - rK).max() <= TOL * np.abs(rK).max(), np.abs(gK - rK).max() / np.abs(rK).max()
+        assert np.abs(gJ.sum(1)).max() < 1e-11 * np.abs(gJ).max() and np.abs(gK.sum(1)).max() < 1e-11 * np.abs(gK).max()
+        # ordered build: K^x(A^T, B) differs from K^x(A, B) for non-symmetric densities (PAPER.md:L85, L164, L308)
+        tJ, tK = gpu_grad(torch, ctx, A.transpose(0, 2, 1).copy(), B)
+        assert np.abs(tK - gK).max() > 1e-3 * np.abs(gK).max()
+        # J-only / K-only outputs
+        Ad, Bd = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+        only = torch.empty((6, ctx.natom, 3), dtype=torch.float64, device="cuda")
+        ctx.jk_grad(Ad, Bd, only, None)
+        torch.cuda.synchronize()
+        assert np.abs(only.cpu().numpy() - gJ).max() <= 1e-12 * np.abs(gJ).max()
+        ctx.close()
+
+
+def test_jk_grad_small_vs_oracle(torch_cuda, small):
+    """N2 at 160 AO (73 contracted s/p/d shells on 14 atoms, 28 M ordered shell quartets): two density pairs against the
+    oracle's product rule (about 3 min of oracle time on the 16 host cores; the kernels take 0.1 s)."""
+    from paper_2607_05622_b200 import ltjk
+    b = small.basis
+    A = random_densities(b.nao, 2, seed=81)
+    B = random_densities(b.nao, 2, seed=82)
+    ctx = ltjk.Context(0)
+    ctx.set_basis(b)
+    gJ, gK = gpu_grad(torch_cuda, ctx, A, B)
+    rJ, rK = O.jk_grad(b, A, B)
+    assert np.abs(gJ - rJ).max() <= TOL * np.abs(rJ).max() and np.abs(gK - rK).max() <= TOL * np.abs(rK).max()
+    assert np.abs(gJ.sum(1)).max() < 1e-11 * np.abs(gJ).max() and np.abs(gK.sum(1)).max() < 1e-11 * np.abs(gK).max()
