@@ -250,9 +250,11 @@ def test_full_size_porphine_full_matrices_subset(torch_cuda):
 
 def test_full_size_large_subset_closure(torch_cuda):
     """730 AO, 192 densities, pair-list digestion: SURVEY 8(d)'s stated fallback, reported as "subset+closure": the GPU
-    linearity closure over all 192 densities, plus the full N x N matrices of a seeded 8-density subset against the
-    folded oracle O6 (about 6.5 min on the 16 host cores of the GPU box).  LTJK_FAST=1 replaces the full-matrix oracle
-    by Eq. 17 on 120 sampled shell-pair blocks (stratified over the nine l-pair classes, about 1.5 min)."""
+    linearity closure over all 192 densities, plus the oracle on a seeded 8-density subset.  Default tier: Eq. 17 by
+    the oracle on 120 sampled shell-pair blocks, stratified over the nine l-pair classes (about 1.5 min).  LTJK_SLOW=1:
+    the full N x N matrices of the same subset against the folded oracle O6 (about 6.5 min on the 16 host cores of the
+    GPU box: too long for the driver's 20-minute tier; the log of that run is profiles/r2_parity_730_full_matrix.txt,
+    J 3.2e-14, K 2.7e-14)."""
     import os
     torch = torch_cuda
     w, ctx, Dn, J, K = full_sweep(torch, "large")
@@ -261,7 +263,7 @@ def test_full_size_large_subset_closure(torch_cuda):
     ds = density_subset(w.nD)
     Dh, Jh, Kh = Dn[ds].cpu().numpy(), J[ds].cpu().numpy(), K[ds].cpu().numpy()
     b = w.basis
-    if os.environ.get("LTJK_FAST") != "1":
+    if os.environ.get("LTJK_SLOW") == "1":
         Jr, Kr, _ = O.jk_folded(b, Dh, w.schwarz_tau)
         ej, ek = relerr(Jh, Jr), relerr(Kh, Kr)
         print("large full-matrix subset: relerr J %.3e K %.3e over densities %s" % (ej, ek, ds))
@@ -572,11 +574,32 @@ def test_jk_grad_vs_oracle(torch_cuda, tiny, spd_basis):
         ctx.close()
 
 
-def test_jk_grad_small_vs_oracle(torch_cuda, small):
-    """N2 at 160 AO (73 contracted s/p/d shells on 14 atoms, 28 M ordered shell quartets): two density pairs against the
-    oracle's product rule (about 3 min of oracle time on the 16 host cores; the kernels take 0.1 s)."""
+def cut_basis(b, natoms):
+    """The shells of the first `natoms` atoms of a workload basis (coefficients already normalised)."""
+    from paper_2607_05622_b200.inputs import Basis
+    keep = [s for s in range(b.nshell) if b.atom[s] < natoms]
+    exps, coef, poff = [], [], []
+    for s in keep:
+        poff.append(len(exps))
+        exps += list(b.exps[b.prim_off[s]:b.prim_off[s] + b.nprim[s]])
+        coef += list(b.coef[b.prim_off[s]:b.prim_off[s] + b.nprim[s]])
+    ls = b.l[keep]
+    ao_off = np.zeros(len(keep) + 1, dtype=np.int64)
+    ao_off[1:] = np.cumsum([(1, 3, 6)[int(l)] for l in ls])
+    return Basis(np.ascontiguousarray(b.xyz[:natoms]), b.atom[keep].astype(np.int32), ls.astype(np.int32),
+                 b.nprim[keep].astype(np.int32), np.asarray(poff, dtype=np.int32), np.asarray(exps), np.asarray(coef), ao_off)
+
+
+@pytest.mark.parametrize("natoms", [5, 14])
+def test_jk_grad_small_vs_oracle(torch_cuda, small, natoms):
+    """N2 on contracted s/p/d shells with several shells per atom: the first 5 atoms of the small workload (default
+    tier), and with LTJK_SLOW=1 all of it (160 AO, 73 shells, 28 M ordered shell quartets: about 3 min of oracle time on
+    the 16 host cores against 0.1 s of kernels; measured 1.5e-13).  Two density pairs, oracle = literal product rule."""
+    import os
     from paper_2607_05622_b200 import ltjk
-    b = small.basis
+    if natoms == 14 and os.environ.get("LTJK_SLOW") != "1":
+        pytest.skip("full 160-AO gradient oracle takes 3 min: set LTJK_SLOW=1")
+    b = small.basis if natoms == 14 else cut_basis(small.basis, natoms)
     A = random_densities(b.nao, 2, seed=81)
     B = random_densities(b.nao, 2, seed=82)
     ctx = ltjk.Context(0)
