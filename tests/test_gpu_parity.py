@@ -608,3 +608,42 @@ def test_jk_grad_small_vs_oracle(torch_cuda, small, natoms):
     rJ, rK = O.jk_grad(b, A, B)
     assert np.abs(gJ - rJ).max() <= TOL * np.abs(rJ).max() and np.abs(gK - rK).max() <= TOL * np.abs(rK).max()
     assert np.abs(gJ.sum(1)).max() < 1e-11 * np.abs(gJ).max() and np.abs(gK.sum(1)).max() < 1e-11 * np.abs(gK).max()
+
+
+def test_pair_list_edge_cases(torch_cuda, tiny):
+    """Degenerate inputs through the pair-list strategy (ltjk_set_digest_mode 2): one density, 200 densities (several
+    column blocks), J-only / K-only, a one-shell basis (a single fully diagonal quartet), a threshold that screens
+    almost everything, and a zero density."""
+    torch = torch_cuda
+    b = tiny.basis
+    ctx = make_ctx(b, mode=2)
+    D = random_densities(b.nao, 200, seed=91)
+    J200, K200 = gpu_jk(torch, ctx, D)
+    Jr, Kr, _ = O.jk_folded(b, D[[0, 137, 199]], tiny.schwarz_tau)
+    assert relerr(J200[[0, 137, 199]], Jr) < TOL and relerr(K200[[0, 137, 199]], Kr) < TOL
+    J1, K1 = gpu_jk(torch, ctx, D[137:138])
+    assert relerr(J1, J200[137:138]) < 1e-12 and relerr(K1, K200[137:138]) < 1e-12
+    Dd = torch.from_numpy(D[:7].copy()).cuda()
+    Jo = torch.full_like(Dd, float("nan"))
+    Ko = torch.full_like(Dd, float("nan"))
+    ctx.jk_build(Dd, Jo, None)
+    ctx.jk_build(Dd, None, Ko)
+    torch.cuda.synchronize()
+    assert relerr(Jo.cpu().numpy(), J200[:7]) < 1e-12 and relerr(Ko.cpu().numpy(), K200[:7]) < 1e-12
+    Z = torch.zeros_like(Dd)
+    ctx.jk_build(Z, Jo, Ko)
+    torch.cuda.synchronize()
+    assert float(Jo.abs().max()) == 0.0 and float(Ko.abs().max()) == 0.0
+    # a threshold that keeps only the strongest quartets: same rule in the oracle (borderline flips are < tau |D|)
+    c2 = make_ctx(b, tau=1e-3, mode=2)
+    Jt, Kt = gpu_jk(torch, c2, D[:3])
+    Jtr, Ktr, kept = O.jk_folded(b, D[:3], 1e-3)
+    assert 0 < kept < b.nshell ** 4 // 8
+    assert relerr(Jt, Jtr) < 1e-9 and relerr(Kt, Ktr) < 1e-9
+    # single d shell on one centre
+    one = custom_basis(np.array([[0.3, -0.1, 0.2]]), [[(2, [0.9, 0.4], [0.6, 0.4])]])
+    c1 = make_ctx(one, tau=0.0, mode=2)
+    D6 = random_densities(6, 2, seed=22)
+    Jg, Kg = gpu_jk(torch, c1, D6)
+    Jd, Kd = O.jk_definition(O.eri_tensor(one), D6)
+    assert relerr(Jg, Jd) < TOL and relerr(Kg, Kd) < TOL
