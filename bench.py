@@ -101,85 +101,98 @@ def pair_integrals(Q, l, tau):
     return out
 
 
-def oracle_sample(w, D, target_s=15.0, nstrata=4):
-    """Time the oracle (as it stands) on a bounded, STRATIFIED sample of the workload: the bra shell-pair list of the
-    folded loop O6 is cut into `nstrata` strata of equal kept-integral share; a run of pairs from the middle of each
-    stratum is timed with all nD densities.  Whole-sweep time = fixed per-call cost + sum_s rate_s x integrals_s: an
-    EXTRAPOLATION (kind says so); the spread of the per-stratum rates is reported."""
-    from oracle import oracle as O
-    b = w.basis
-    Q = O.schwarz(b)
-    npair = b.nshell * (b.nshell + 1) // 2
-    pints = pair_integrals(Q, b.l, w.schwarz_tau)
-    cum = np.concatenate([[0.0], np.cumsum(pints)])
-    total_ints = float(cum[-1])
+class OracleSampler:
+    """Times the oracle (as it stands) on bounded, STRATIFIED samples of the workload.  The bra shell-pair list of the
+    folded loop O6 is cut into `nstrata` strata of equal kept-integral share; a sample is a run of bra pairs from the
+    middle of one stratum, timed with all nD densities.  The oracle threads over bra pairs, so a run holds as many
+    pairs as there are cores (a shorter run would leave cores idle and understate its rate).  Whole-sweep time =
+    fixed per-call cost + sum_s rate_s x integrals_s: an EXTRAPOLATION, labelled so."""
 
-    def call(pa, pb):
+    def __init__(self, w, D, nstrata=4):
+        from oracle import oracle as O
+        self.O, self.w, self.D, self.nstrata = O, w, D, nstrata
+        b = w.basis
+        self.Q = O.schwarz(b)
+        self.npair = b.nshell * (b.nshell + 1) // 2
+        pints = pair_integrals(self.Q, b.l, w.schwarz_tau)
+        self.cum = np.concatenate([[0.0], np.cumsum(pints)])
+        self.total = float(self.cum[-1])
+        self.ncores = O.max_threads()
+        self.mids = [int(np.searchsorted(self.cum, self.total * (k + 0.5) / nstrata)) for k in range(nstrata)]
+        self.bounds = [int(np.searchsorted(self.cum, self.total * k / nstrata)) for k in range(nstrata + 1)]
+        self.bounds[0], self.bounds[-1] = 0, self.npair
+        self.used = 0.0
+        self.t_fixed = self.call(0, 0)     # density-fastest copies of D, per-thread J/K buffers and their reduction
+        self.rates = [[] for _ in range(nstrata)]
+        self.sampled = 0.0
+
+    def call(self, pa, pb):
         t = time.perf_counter()
-        O.jk_folded(b, D, w.schwarz_tau, pair_range=(pa, pb), Q=Q)
-        return time.perf_counter() - t
+        self.O.jk_folded(self.w.basis, self.D, self.w.schwarz_tau, pair_range=(pa, pb), Q=self.Q)
+        dt = time.perf_counter() - t
+        self.used += dt
+        return dt
 
-    t_fixed = call(0, 0)                   # density-fastest copies of D, per-thread J/K buffers and their reduction
-    bounds = [int(np.searchsorted(cum, total_ints * k / nstrata)) for k in range(nstrata + 1)]
-    bounds[0], bounds[-1] = 0, npair
-    mids = [int(np.searchsorted(cum, total_ints * (k + 0.5) / nstrata)) for k in range(nstrata)]
-    # calibration: a short run in the first stratum sizes the samples to the time budget
-    pa = min(mids[0], npair - 1)
-    t_cal = call(pa, min(pa + 2, npair))
-    rate_cal = max(t_cal - t_fixed, 1e-3) / max(cum[min(pa + 2, npair)] - cum[pa], 1.0)
-    per = max((target_s - 2 * t_fixed - t_cal) / nstrata - t_fixed, 0.5)
-    rates, used, sampled = [], t_fixed + t_cal, 0.0
+    def sample(self, k):
+        pa = min(self.mids[k], max(self.npair - self.ncores, 0))
+        pb = min(pa + self.ncores, self.npair)
+        t = self.call(pa, pb)
+        ints = max(self.cum[pb] - self.cum[pa], 1.0)
+        self.rates[k].append(max(t - self.t_fixed, 1e-6) / ints)
+        self.sampled += ints
+        return t
+
+    def result(self):
+        known = [float(np.mean(r)) for r in self.rates if r]
+        per = [float(np.mean(r)) if r else float(np.mean(known)) for r in self.rates]
+        strata_ints = [self.cum[self.bounds[k + 1]] - self.cum[self.bounds[k]] for k in range(self.nstrata)]
+        sweep_s = self.t_fixed + float(sum(r * n for r, n in zip(per, strata_ints)))
+        allr = [x for r in self.rates for x in r]
+        return {"value": self.D.shape[0] / sweep_s, "unit": UNIT, "cores": self.ncores,
+                "kind": "oracle (extrapolated from a stratified bounded sample)", "extrapolated": True,
+                "cpu_seconds_spent": self.used, "rate_s_per_integral": {"min": min(allr), "max": max(allr)},
+                "sample": "oracle O6 (folded MD loop, all %d densities): %.1f s of CPU time; fixed cost per call %.2f s "
+                          "(empty pair range); %d strata of equal integral share, %d run(s) of %d bra shell pairs from "
+                          "the middle of a stratum: %.3g of the %.3g kept unique integrals sampled, %.3g-%.3g s per "
+                          "integral; sweep = fixed + sum_s rate_s x integrals_s" %
+                          (self.D.shape[0], self.used, self.t_fixed, self.nstrata, len(allr), self.ncores, self.sampled,
+                           self.total, min(allr), max(allr))}
+
+
+def oracle_sample(w, D, nstrata=4):
+    smp = OracleSampler(w, D, nstrata)
     for k in range(nstrata):
-        pa = min(mids[k], npair - 1)
-        pb = int(np.searchsorted(cum, cum[pa] + per / rate_cal))
-        pb = max(pa + 1, min(pb, bounds[k + 1], npair))
-        t = call(pa, pb)
-        ints = max(cum[pb] - cum[pa], 1.0)
-        rates.append(max(t - t_fixed, 1e-6) / ints)
-        used += t
-        sampled += ints
-    strata_ints = [cum[bounds[k + 1]] - cum[bounds[k]] for k in range(nstrata)]
-    sweep_s = t_fixed + float(sum(r * n for r, n in zip(rates, strata_ints)))
-    return {"value": D.shape[0] / sweep_s, "unit": UNIT, "cores": O.max_threads(),
-            "kind": "oracle (extrapolated from a stratified bounded sample)", "extrapolated": True,
-            "cpu_seconds_spent": used, "rate_s_per_integral": {"min": min(rates), "max": max(rates)},
-            "sample": "oracle O6 (folded MD loop, all %d densities): %.1f s of CPU time; fixed cost per call %.2f s "
-                      "(empty pair range); %d strata of equal integral share, one run of bra shell pairs from the "
-                      "middle of each: %.3g of the %.3g kept unique integrals sampled, %.3g-%.3g s per integral; "
-                      "sweep = fixed + sum_s rate_s x integrals_s" %
-                      (D.shape[0], used, t_fixed, nstrata, sampled, total_ints, min(rates), max(rates))}
+        smp.sample(k)
+    return smp.result()
 
 
 def run_reference(args, rank, world):
-    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only).  Each step is one bounded,
-    stratified sample of the workload; `ms_per_step` is the wall time the step really took, `value` the whole-sweep
-    rate extrapolated from the samples (flagged)."""
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only).  Each step times one bounded sample
+    (a run of bra shell pairs from one stratum, strata visited in turn); `ms_per_step` is the wall time a step really
+    took, `value` the whole-sweep rate extrapolated from the timed samples (flagged)."""
     if rank != 0:
         return
-    from oracle import oracle as O
     from paper_2607_05622_b200.inputs import make_workload
     w = make_workload(args.workload)
     nD = w.nD
     rng = np.random.default_rng(1)
     D = 1e-2 * rng.standard_normal((nD, w.nao, w.nao))    # cost does not depend on the values (PAPER.md:L565)
-    per = max(4.0, min(20.0, 150.0 / max(args.steps + args.warmup, 1)))
-    vals, walls = [], []
-    for s in range(args.warmup + args.steps):
-        t0 = time.perf_counter()
-        r = oracle_sample(w, D, target_s=per)
-        if s >= args.warmup:
-            vals.append(r)
-            walls.append(time.perf_counter() - t0)
-    v = float(np.mean([r["value"] for r in vals]))
+    smp = OracleSampler(w, D)
+    for s in range(args.warmup):
+        smp.sample(s % smp.nstrata)
+    smp.rates = [[] for _ in range(smp.nstrata)]
+    smp.sampled = 0.0
+    walls = [smp.sample(s % smp.nstrata) for s in range(args.steps)]
+    r = smp.result()
+    v = r["value"]
     out = {"impl": "reference", "metric": metric_name(w), "value": v, "unit": UNIT, "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(walls)),
            "ms_per_step_is": "wall time of one bounded sample step (NOT of a whole sweep)",
            "extrapolated": True, "extrapolated_ms_per_sweep": 1e3 * nD / v,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": "%s (%d AO, %d densities)" % (w.name, w.nao, nD), "tau_schwarz": w.schwarz_tau},
-           "cpu_baseline": {"value": v, "unit": UNIT, "cores": vals[-1]["cores"], "kind": vals[-1]["kind"],
-                            "sample": vals[-1]["sample"],
-                            "spread_over_steps": [min(r["value"] for r in vals), max(r["value"] for r in vals)]},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": r["cores"], "kind": r["kind"], "sample": r["sample"],
+                            "rate_s_per_integral": r["rate_s_per_integral"]},
            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(out), flush=True)
 
@@ -411,7 +424,7 @@ def main():
                      frac_of_f64_tensor_peak=rep["transform"]["tflops"] / f64_tensor_peak)
     cpu = None
     if not args.no_cpu_baseline:
-        cpu = oracle_sample(w, Dn.cpu().numpy(), target_s=20.0)
+        cpu = oracle_sample(w, Dn.cpu().numpy())
     launches = int(rep["launches_per_step"] * args.steps)
     e2e = None
     if "ms_e2e" in rep:
