@@ -246,6 +246,7 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
     int TN, nb;
     digest_colblocks(nD, c->digest_mode, &TN, &nb);
     const int nDp = TN * nb * 32;
+    c->cur_nD = nD;
     int rc;
     if ((rc = ensure_work(c, nDp))) return rc;
     c->st_launches = 0; c->st_quartets = 0; c->st_digest_flops = 0.0;

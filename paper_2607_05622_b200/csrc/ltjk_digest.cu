@@ -35,6 +35,7 @@ struct DigestArgs {
     double* Jt;
     double* Kt;
     int nDp;
+    int fuse;                    // nD <= 16 (TN = 1): the two partners of a K item share one pass, 16 columns each
 };
 
 template <int TN>
@@ -47,6 +48,7 @@ struct DigestSmem {
     int rowoff[kMT];
     int acol[kMaxNC];
     unsigned bcol[kMaxNC];
+    unsigned bcol2[kMaxNC];              // fused partner (g.fuse): density row of the transposed partner
 };
 
 
@@ -119,6 +121,8 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
             const ItemCtx c = load_item(g, vi, ncolblk, 32 * TN);
             const DigestItem& it = c.it;
             const int view = it.view, I = c.sc.I, J = c.sc.J, nI = c.nI, nJ = c.nJ;
+            const bool fused = (TN == 1) && g.fuse && view >= 2;    // both partners of a K item in one pass
+            if (fused && it.partner) continue;                      // done by its partner-0 twin (same tile, same mask)
             const bool partner = it.partner != 0;
             const double* __restrict__ Bmat = (view <= 1) ? g.Dst : g.Dt;
             const bool rowContig = (view == 1 || view >= 4);   // l (unit stride) is a row index
@@ -149,6 +153,7 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
                     const int c1 = cidx / nC2, c2 = cidx % nC2;
                     S.acol[cidx] = c1 * sC1 + c2 * sC2;
                     S.bcol[cidx] = partner ? (unsigned)((aoC2 + c2) * N + aoC1 + c1) : (unsigned)((aoC1 + c1) * N + aoC2 + c2);
+                    if (fused) S.bcol2[cidx] = (unsigned)((aoC2 + c2) * N + aoC1 + c1);
                 }
                 asm volatile("bar.sync 1, %0;\n" ::"n"(kProducerThreads));
                 const int nch = (nC + kKC - 1) / kKC;
@@ -184,8 +189,15 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
                         const int k = pw + kProducerWarps * h, cidx = ch * kKC + k;
                         const bool ok = cidx < nC;
                         const double* src = ok ? (Bmat + (size_t)S.bcol[cidx] * nDp + c.n0) : Bmat;
-                        for (int pc = lane; pc < 16 * TN; pc += 32)
-                            cp_async16(&S.B[st][k][pc * 2], src + (ok ? pc * 2 : 0), ok);
+                        if (fused) {
+                            // columns 0..15: densities of partner 0;  columns 16..31: the same densities, partner 1
+                            const double* src2 = ok ? (Bmat + (size_t)S.bcol2[cidx] * nDp + c.n0) : Bmat;
+                            if (lane < 16)
+                                cp_async16(&S.B[st][k][lane * 2], (lane < 8 ? src : src2) + (ok ? (lane & 7) * 2 : 0), ok);
+                        } else {
+                            for (int pc = lane; pc < 16 * TN; pc += 32)
+                                cp_async16(&S.B[st][k][pc * 2], src + (ok ? pc * 2 : 0), ok);
+                        }
                     }
                     mbar_arrive_on_cp_async(&S.full[st]);
                     if (pt == 0) { S.cmask[st] = wbits; mbar_arrive(&S.full[st]); }   // release: visible after the wait
@@ -209,6 +221,8 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
         const ItemCtx c = load_item(g, vi, ncolblk, 32 * TN);
         const DigestItem& it = c.it;
         const int view = it.view;
+        const bool fused = (TN == 1) && g.fuse && view >= 2;
+        if (fused && it.partner) continue;
         const int total_chunks = it.nnz;
         const bool warp_active = it.rowtile * kMT + wrow < c.nrows;   // ragged last tile: idle warps skip the DFMAs
         double acc[8][2 * TN];
@@ -254,8 +268,10 @@ __global__ void __launch_bounds__(kDigestThreads, 1) digest_kernel(const DigestA
                 const int m = it.rowtile * kMT + trow + r;
                 if (m < c.nrows) {
                     const int r1 = m / c.nR2, r2 = m % c.nR2;
-                    const size_t row = partner ? (size_t)(aoR2 + r2) * N + aoR1 + r1 : (size_t)(aoR1 + r1) * N + aoR2 + r2;
-                    double* o = Out + row * nDp + c.n0 + 2 * l16;
+                    // fused: lanes 8..15 of a half-warp hold partner 1 -> transposed output row, densities 2 (l16 - 8)
+                    const bool tr = fused ? (l16 >= 8) : partner;
+                    const size_t row = tr ? (size_t)(aoR2 + r2) * N + aoR1 + r1 : (size_t)(aoR1 + r1) * N + aoR2 + r2;
+                    double* o = Out + row * nDp + c.n0 + 2 * (fused ? (l16 & 7) : l16);
 #pragma unroll
                     for (int t = 0; t < TN; ++t) {
                         atomicAdd(o + 32 * t, mult * acc[r][2 * t]);
@@ -374,6 +390,7 @@ int launch_digest(ltjk_ctx* c, const Group& ch, int nDp, bool doJ, bool doK)
     g.nDp = nDp;
     int TN, nb;
     digest_colblocks(nDp, 1, &TN, &nb);
+    g.fuse = (TN == 1 && nb == 1 && c->cur_nD <= 16) ? 1 : 0;
     if (nb * TN * 32 != nDp) return set_err(c, LTJK_EINVAL, "internal: nDp is not a whole number of column blocks");
     c->st_launches++;
     switch (TN) {
