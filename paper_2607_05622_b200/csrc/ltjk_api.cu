@@ -237,6 +237,10 @@ int ltjk_create(ltjk_ctx** out, int device, void* cuda_stream)
     std::vector<double> tab = make_boys_table(kBoysNT, kBoysNM);
     if (cudaMalloc(&c->t.boys, sizeof(double) * tab.size()) != cudaSuccess ||
         cudaMemcpy(c->t.boys, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+        if (c->t.boys) cudaFree(c->t.boys);
+        for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_eri[i]); cudaEventDestroy(c->ev_dig[i]); }
+        cudaEventDestroy(c->ev_start);
+        cudaStreamDestroy(c->own_stream);
         delete c;
         return LTJK_ECUDA;
     }

@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <initializer_list>
 
 using namespace ltjk;
 
@@ -256,6 +257,10 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
     if (J) LTJK_CUDA(c, cudaMemsetAsync(c->Jt, 0, wbytes, c->stream));
     if (K) LTJK_CUDA(c, cudaMemsetAsync(c->Kt, 0, wbytes, c->stream));
     cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
+    struct EvGuard {            // timing events are released on every exit path (early error returns included)
+        cudaEvent_t *a, *b, *c;
+        ~EvGuard() { for (cudaEvent_t* e : {a, b, c}) if (*e) { cudaEventDestroy(*e); *e = nullptr; } }
+    } evguard{&e0, &e1, &e2};
     if (c->timing) { cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventCreate(&e2); }
     if (c->digest_mode == 2) {
         // pair-list pipeline: per chunk, clear its ring half, generate the integrals of the chunk under all role
@@ -299,7 +304,6 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
             c->st_digest_flops += 2.0 * nDp * ((J ? ch.exec_rows_chunks_J : 0.0) + (K ? ch.exec_rows_chunks_K : 0.0));
         }
         c->st_quartets = c->n_quartets_kept;
-        if (c->timing) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2); }
         if ((rc = launch_unpack_results(c, nD, nDp, J, K))) return rc;
         return LTJK_OK;
     }
@@ -345,7 +349,6 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
         c->st_quartets += gr.nquartets;
         c->st_digest_flops += 2.0 * gr.nints * nDp * ((J ? 2.0 : 0.0) + (K ? 8.0 : 0.0));   // images applied (folded ones included)
     }
-    if (c->timing) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2); }
     if (c->resident) c->panels_valid = true;            // the panels of this geometry stay in HBM for the next build
     if ((rc = launch_unpack_results(c, nD, nDp, J, K))) return rc;
     return LTJK_OK;
