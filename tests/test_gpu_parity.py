@@ -246,6 +246,11 @@ def test_full_size_porphine_full_matrices_subset(torch_cuda):
     Jr, Kr, _ = O.jk_folded(w.basis, Dn[ds].cpu().numpy(), w.schwarz_tau)
     assert relerr(J[ds].cpu().numpy(), Jr) < TOL and relerr(K[ds].cpu().numpy(), Kr) < TOL
     linearity_closure(torch_cuda, ctx, Dn, J, K)
+    # the same sweep forced onto the pair-list strategy (3 shell groups at this size) against the same oracle result
+    del ctx, J, K
+    w2, ctx2, Dn2, J2, K2 = full_sweep(torch_cuda, "porphine", mode=2)
+    assert ctx2.get_digest_mode() == 2
+    assert relerr(J2[ds].cpu().numpy(), Jr) < TOL and relerr(K2[ds].cpu().numpy(), Kr) < TOL
 
 
 def test_full_size_large_subset_closure(torch_cuda):
