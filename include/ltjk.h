@@ -201,6 +201,12 @@ int ltjk_set_resident(ltjk_ctx* ctx, int enable);
 /* The strategy (1 or 2) chosen by the last ltjk_build_shell_pairs; LTJK_ENOBASIS before it. */
 int ltjk_get_digest_mode(const ltjk_ctx* ctx, int* mode);
 
+/* Test hook (compute-sanitizer is not available on every GPU pool): with enable != 0 every ltjk_jk_build fills the
+ * integral staging ring with NaN before each launch unit, so that an element the digestion reads but neither an ERI
+ * kernel nor the zero fill wrote -- stale data of an earlier unit would otherwise hide it -- turns the result into
+ * NaN.  Slower; results are unchanged when the write coverage is complete. */
+int ltjk_debug_poison(ltjk_ctx* ctx, int enable);
+
 /* Test hook: contracted Cartesian shell quartet (A B|C D) in the caller's shell indices, evaluated by the
  * device ERI kernel, written to HOST out[na*nb*nc*nd] (row-major a,b,c,d).  Synchronises. */
 int ltjk_debug_eri_quartet(ltjk_ctx* ctx, int A, int B, int C, int D, double* out_host);

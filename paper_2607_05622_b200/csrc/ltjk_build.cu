@@ -284,6 +284,8 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
             if (!c->timing && used[ch.buf]) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[ch.buf], 0));
             used[ch.buf] = true;
             if (c->timing) cudaEventRecord(e0, c->stream);
+            if (c->debug_poison)     // every element the digestion reads must be written by pzero or an ERI kernel
+                LTJK_CUDA(c, cudaMemsetAsync(c->d_pring + (size_t)ch.buf * c->pring_half, 0xFF, sizeof(double) * ch.doubles, c->eri_stream));
             if ((rc = launch_pzero(c, ch))) return rc;
             if ((rc = launch_peri_chunk(c, ch))) return rc;
             if (c->timing) cudaEventRecord(e1, c->stream);
@@ -328,6 +330,8 @@ int ltjk_jk_build(ltjk_ctx* c, int nD, const double* D, double* J, double* K)
         if (!c->timing && !c->resident && used[gr.buf]) LTJK_CUDA(c, cudaStreamWaitEvent(c->eri_stream, c->ev_dig[gr.buf], 0));
         used[gr.buf] = true;
         if (c->timing) cudaEventRecord(e0, c->stream);
+        if (c->debug_poison && !c->resident)
+            LTJK_CUDA(c, cudaMemsetAsync(c->d_panel + (size_t)gr.buf * c->panel_half, 0xFF, sizeof(double) * c->panel_half, c->eri_stream));
         if (!(c->resident && c->panels_valid))
             for (int ck = 0; ck <= gr.cb; ++ck)
                 if ((rc = launch_eri_panels(c, gr, ck))) return rc;
@@ -510,6 +514,13 @@ int ltjk_set_quartet_shard(ltjk_ctx* c, int rank, int world)
     if (!c || world < 1 || rank < 0 || rank >= world) return LTJK_EINVAL;
     if (rank != c->shard_rank || world != c->shard_world) c->panels_valid = false;   // resident panels: other units now
     c->shard_rank = rank; c->shard_world = world;
+    return LTJK_OK;
+}
+
+int ltjk_debug_poison(ltjk_ctx* c, int enable)
+{
+    if (!c) return LTJK_EINVAL;
+    c->debug_poison = enable != 0;
     return LTJK_OK;
 }
 

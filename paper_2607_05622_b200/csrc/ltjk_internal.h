@@ -186,6 +186,7 @@ struct ltjk_ctx {
     double *gr_xyz = nullptr, *gr_exps = nullptr, *gr_coef = nullptr;   // basis in caller order for ltjk_jk_grad (ltjk_grad.cu)
     int* gr_int = nullptr;
     int gr_cnt[3] = {0, 0, 0};
+    bool debug_poison = false;             // test hook: the staging ring is filled with NaN before every chunk / group
     int cur_nD = 0;                        // density count of the build in progress (un-padded)
     int shard_rank = 0, shard_world = 1;   // quartet-space split of one build over ranks (ltjk_set_quartet_shard)
     double* na_scratch = nullptr;          // device address of the static no-allocation scratch (ltjk_transform.cu), per device

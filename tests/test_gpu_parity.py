@@ -652,3 +652,26 @@ def test_pair_list_edge_cases(torch_cuda, tiny):
     Jg, Kg = gpu_jk(torch, c1, D6)
     Jd, Kd = O.jk_definition(O.eri_tensor(one), D6)
     assert relerr(Jg, Jd) < TOL and relerr(Kg, Kd) < TOL
+
+
+@pytest.mark.parametrize("name,mode,scratch", [("small", 1, 1 << 20), ("small", 2, 1 << 22), ("medium", 1, None),
+                                               ("medium", 2, None), ("large", 2, None)])
+def test_staging_ring_write_coverage(torch_cuda, name, mode, scratch):
+    """Stand-in for a memory checker (compute-sanitizer is closed on this pool): with ltjk_debug_poison the staging ring
+    is NaN before every launch unit, so any element the digestion reads that neither an ERI kernel nor the zero fill
+    wrote -- which stale integrals of an earlier unit would hide -- makes J or K NaN.  The poisoned build must be
+    finite and equal to the normal one (same kernels, same order: tight tolerance); 730 AO covers 55 chunks of 5 groups."""
+    torch = torch_cuda
+    w = make_workload(name)
+    ctx = make_ctx(w.basis, scratch=scratch, mode=mode)
+    nD = 3 if name != "large" else 2
+    D = torch.from_numpy(random_densities(w.nao, nD, seed=95)).cuda()
+    J0, K0 = torch.empty_like(D), torch.empty_like(D)
+    ctx.jk_build(D, J0, K0)
+    ctx.debug_poison(True)
+    J1, K1 = torch.full_like(D, 1.0), torch.full_like(D, 1.0)
+    ctx.jk_build(D, J1, K1)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(J1).all()) and bool(torch.isfinite(K1).all())
+    assert float((J1 - J0).abs().max()) <= 1e-12 * float(J0.abs().max())
+    assert float((K1 - K0).abs().max()) <= 1e-12 * float(K0.abs().max())
