@@ -675,3 +675,28 @@ def test_staging_ring_write_coverage(torch_cuda, name, mode, scratch):
     assert bool(torch.isfinite(J1).all()) and bool(torch.isfinite(K1).all())
     assert float((J1 - J0).abs().max()) <= 1e-12 * float(J0.abs().max())
     assert float((K1 - K0).abs().max()) <= 1e-12 * float(K0.abs().max())
+
+
+@pytest.mark.parametrize("mode,scratch", [(1, 1 << 20), (2, 1 << 22)])
+def test_ring_reuse_stress(torch_cuda, small, mode, scratch):
+    """Two-stream pipeline with a tiny staging ring (dozens of launch units alternate between the two ring halves; the
+    ERI kernels of unit g+1 run while unit g is digested): 12 back-to-back builds without any host synchronisation in
+    between must all agree with the first one (fp64 reductions reorder: 1e-12) and with the oracle -- a ring half
+    overwritten too early, or read too early, shows up here."""
+    torch = torch_cuda
+    w = small
+    D = random_densities(w.nao, 5, seed=97)
+    Jr, Kr, _ = O.jk_folded(w.basis, D, w.schwarz_tau)
+    ctx = make_ctx(w.basis, scratch=scratch, mode=mode)
+    Dd = torch.from_numpy(D).cuda()
+    outs = []
+    for _ in range(12):
+        J = torch.empty_like(Dd)
+        K = torch.empty_like(Dd)
+        ctx.jk_build(Dd, J, K)
+        outs.append((J, K))
+    torch.cuda.synchronize()
+    J0, K0 = outs[0][0].cpu().numpy(), outs[0][1].cpu().numpy()
+    assert relerr(J0, Jr) < TOL and relerr(K0, Kr) < TOL
+    for J, K in outs[1:]:
+        assert relerr(J.cpu().numpy(), J0) < 1e-12 and relerr(K.cpu().numpy(), K0) < 1e-12
