@@ -27,8 +27,11 @@
  *   orc_jk_grad            SURVEY 8(f) N2: derivative builds J^x(A,B), K^x(A,B), Eq. (18), written out
  *                          term by term (one term per differentiated function), no symmetry used
  *
+ * Input shells: Cartesian s, p, d, f (f: SURVEY.md 8(f) row N4); orc_jk_grad: s, p, d.
+ *
  * Pins (tests/test_oracle_*.py): Boys vs mpmath quadrature / gammainc / closed forms; (ss|ss) closed form,
- * 2 sqrt(a/pi), erf(sqrt(rho) R)/R; finite differences in the centre for p and d; 8-fold symmetry of O7;
+ * 2 sqrt(a/pi), erf(sqrt(rho) R)/R; centre derivatives of the closed-form (ss|ss) in 150-198 digit arithmetic for
+ * sampled components of every class family up to (dd|dd) and of the f classes up to (ff|ff); 8-fold symmetry of O7;
  * Cauchy-Schwarz, PSD; translation/rotation invariance; O6 vs O7; J/K symmetry relations; orc_jk_grad: central finite
  * differences of tr(A^T J[B]), tr(A^T K[B]) built from orc_eri_tensor, closed form d/dR [erf(sqrt(rho) R)/R], the
  * translational sum rule Eq. (31), J^x(A,B) = J^x(B,A), K^x(A,B) = K^x(B,A) = K^x(A^T,B^T)  (tests/test_oracle_grad.py).
@@ -39,12 +42,14 @@
 #include <string.h>
 #include <omp.h>
 
-#define LMAXSH 2                   /* largest angular momentum of an input shell */
-#define LMAXW 3                    /* largest angular momentum inside eri_shell: the derivative builds (orc_jk_grad) raise ONE index by one */
-#define LTOT (3 * LMAXSH + LMAXW)  /* 9 */
+#define LMAXSH 3                   /* largest angular momentum of an input shell of the value builds (s, p, d, f; row N4) */
+#define LMAXW 3                    /* largest angular momentum inside eri_shell: f input shells, or the derivative builds
+                                      (orc_jk_grad, input shells l <= 2 only) raising ONE index by one */
+#define LTOT (4 * LMAXW)           /* 12 */
 #define NH1 (2 * LMAXW + 1)        /* Hermite orders per pair and dimension */
-#define NR (LTOT + 1)              /* 10 */
+#define NR (LTOT + 1)              /* 13 */
 #define NCMAX 10                   /* Cartesian components of an l = LMAXW shell */
+#define NQMAX (NCMAX * NCMAX * NCMAX * NCMAX)   /* integrals of one (ff|ff) shell quartet */
 
 static const double PI = 3.14159265358979323846264338327950288;
 
@@ -258,7 +263,7 @@ void orc_eri_tensor(BASIS_ARGS, double *eri)
     long N = off[nshell];
 #pragma omp parallel
     {
-        double *buf = (double *)malloc(sizeof(double) * 1296);
+        double *buf = (double *)malloc(sizeof(double) * NQMAX);
 #pragma omp for collapse(2) schedule(dynamic)
         for (int A = 0; A < nshell; ++A)
         for (int B = 0; B < nshell; ++B)
@@ -282,7 +287,7 @@ void orc_schwarz(BASIS_ARGS, double *Q)
     basis_t bs = BASIS_INIT;
 #pragma omp parallel
     {
-        double *buf = (double *)malloc(sizeof(double) * 1296);
+        double *buf = (double *)malloc(sizeof(double) * NQMAX);
 #pragma omp for schedule(dynamic)
         for (int A = 0; A < nshell; ++A)
             for (int B = 0; B <= A; ++B) {
@@ -331,7 +336,7 @@ long long orc_jk_folded(BASIS_ARGS, double tau, int nD, const double *D, double 
     {
         int tid = omp_get_thread_num();
         double *Jp = Jt + sz * tid, *Kp = Kt + sz * tid;
-        double *buf = (double *)malloc(sizeof(double) * 1296);
+        double *buf = (double *)malloc(sizeof(double) * NQMAX);
 #pragma omp for schedule(dynamic)
         for (long long ab = pair_begin; ab < pair_end; ++ab) {
             int A = (int)((sqrt(8.0 * (double)ab + 1.0) - 1.0) / 2.0);
@@ -405,7 +410,7 @@ void orc_jk_blocks(BASIS_ARGS, double tau, int nD, const double *D, int nblk, co
         for (long i = 0; i < (long)nD * nx * ny; ++i) Jo[i] = Ko[i] = 0.0;
 #pragma omp parallel
         {
-            double *buf = (double *)malloc(sizeof(double) * 1296);
+            double *buf = (double *)malloc(sizeof(double) * NQMAX);
             double *jl = (double *)calloc((size_t)nD * nx * ny, sizeof(double));
             double *kl = (double *)calloc((size_t)nD * nx * ny, sizeof(double));
 #pragma omp for collapse(2) schedule(dynamic)

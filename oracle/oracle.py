@@ -84,7 +84,7 @@ def boys(mmax: int, T: float) -> np.ndarray:
     return F
 
 
-_NC = (1, 3, 6)
+_NC = (1, 3, 6, 10)
 
 
 def eri_shell(b, A, B, C, D) -> np.ndarray:
@@ -160,6 +160,8 @@ def jk_grad(b, A: np.ndarray, B: np.ndarray):
     """J^x(A,B), K^x(A,B) of Eq. (18) for nP density pairs; returns two arrays
     [nP, natom, 3].  Plain product rule over the four functions of every ordered shell quartet (orc_jk_grad)."""
     args, keep = _basis_args(b)
+    if int(np.max(np.asarray(b.l))) > 2:
+        raise ValueError("jk_grad: the derivative oracle raises one index by one and is sized for input shells l <= 2")
     A = np.ascontiguousarray(A, dtype=np.float64)
     B = np.ascontiguousarray(B, dtype=np.float64)
     nP = A.shape[0]

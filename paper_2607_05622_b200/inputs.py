@@ -24,7 +24,7 @@ SEED0 = 20260705
 LAPLACE_RANGE = (0.4, 4.5)  # denominators x = eps_a - eps_i lie in [0.4, 4.5] E_h
 SCHWARZ_TAU = 1e-12
 
-NCART = (1, 3, 6)
+NCART = (1, 3, 6, 10)
 
 
 def _dfact2lm1(l: int) -> float:

@@ -15,7 +15,8 @@ from oracle import oracle as O
 from paper_2607_05622_b200.inputs import custom_basis, prim_norm
 
 CART = {0: [(0, 0, 0)], 1: [(1, 0, 0), (0, 1, 0), (0, 0, 1)],
-        2: [(2, 0, 0), (1, 1, 0), (1, 0, 1), (0, 2, 0), (0, 1, 1), (0, 0, 2)]}
+        2: [(2, 0, 0), (1, 1, 0), (1, 0, 1), (0, 2, 0), (0, 1, 1), (0, 0, 2)],
+        3: [(3, 0, 0), (2, 1, 0), (2, 0, 1), (1, 2, 0), (1, 1, 1), (1, 0, 2), (0, 3, 0), (0, 2, 1), (0, 1, 2), (0, 0, 3)]}
 
 
 def ssss_closed(a, b, c, d, A, B, C, D):
@@ -42,6 +43,8 @@ def _dir_terms(n, a):
         return [(1 / (2 * a), 1)]
     if n == 2:
         return [(1 / (4 * a * a), 2), (1 / (2 * a), 0)]
+    if n == 3:      # d^3 = (8 a^3 x^3 - 12 a^2 x) e  and  x e = d / (2a)
+        return [(1 / (8 * a ** 3), 3), (3 / (4 * a * a), 1)]
     raise ValueError
 
 
@@ -55,6 +58,8 @@ def _fd_partial(f, x0, orders, h):
             stencils.append([(1, 1 / (2 * h)), (-1, -1 / (2 * h))])
         elif n == 2:
             stencils.append([(1, 1 / h ** 2), (0, -2 / h ** 2), (-1, 1 / h ** 2)])
+        elif n == 3:
+            stencils.append([(2, 1 / (2 * h ** 3)), (1, -1 / h ** 3), (-1, 1 / h ** 3), (-2, -1 / (2 * h ** 3))])
         else:
             raise ValueError
     tot = mp.mpf(0)
@@ -72,8 +77,10 @@ def _fd_partial(f, x0, orders, h):
 def cart_eri_by_differentiation(expo, cents, comps):
     """Unnormalised primitive Cartesian ERI via centre-derivatives of the closed-form (ss|ss).
 
-    150-digit arithmetic, h = 1e-12: truncation error O(h^2) ~ 1e-24 relative, cancellation <= 96 digits."""
-    mp.mp.dps = 150
+    h = 1e-12: truncation error O(h^2) ~ 1e-24 relative; the cancellation is 12 digits per derivative order, so the
+    working precision is 54 digits above that (150 digits up to (dd|dd), 198 for (ff|ff))."""
+    order = sum(sum(c) for c in comps)
+    mp.mp.dps = max(150, 54 + 12 * order)
     h = mp.mpf(10) ** (-12)
     expo = [mp.mpf(e) for e in expo]
     x0 = [mp.mpf(float(v)) for cen in cents for v in cen]
@@ -146,9 +153,15 @@ CLASSES = [(1, 0, 0, 0), (0, 1, 0, 0), (0, 0, 1, 0), (0, 0, 0, 1), (1, 1, 0, 0),
            (2, 0, 2, 0), (2, 1, 2, 1), (1, 2, 1, 0), (2, 2, 1, 1), (2, 2, 2, 1), (2, 2, 2, 2)]
 
 
-@pytest.mark.parametrize("ls", CLASSES)
+# classes with f shells: f in every position, next to every other l, up to (ff|ff)
+CLASSES_F = [(3, 0, 0, 0), (0, 3, 0, 0), (0, 0, 3, 0), (0, 0, 0, 3), (3, 1, 0, 0), (1, 3, 2, 0), (3, 0, 3, 0),
+             (3, 3, 0, 0), (3, 2, 3, 1), (2, 3, 1, 3), (3, 3, 2, 2), (3, 3, 3, 3)]
+
+
+@pytest.mark.parametrize("ls", CLASSES + CLASSES_F)
 def test_cartesian_classes_by_differentiating_closed_form(ls):
-    """Every angular class up to (dd|dd): sampled components vs derivatives of the closed-form (ss|ss)."""
+    """Every angular class up to (dd|dd), and the f classes up to (ff|ff): sampled components vs derivatives of the
+    closed-form (ss|ss)."""
     rng = np.random.default_rng(100 + sum(k * 3 ** i for i, k in enumerate(ls)))
     cents = rng.uniform(-1.2, 1.2, size=(4, 3))
     expo = list(rng.uniform(0.4, 1.6, size=4))
