@@ -6,10 +6,13 @@
 * O10 pseudo-density as explicit loops                                            PAPER.md:L136-145 Eqs. (13),(15)
 
 * N1 laplace_fock / laplace_accumulate (Eqs. (19), (21)), N3 pp_ladder
+* N4 sph_matrix / sph_from_cart / cart_from_sph: the spherical-harmonic transform at matrix level
 
 Pins (tests/test_oracle_*.py, CPU tier): O9 equi-oscillation certificate, scaling law, Lawson cross-check; O10 tau = 0
 product, rank-1 Eq. (14) case, unit amplitudes, layout, denominator resolution with the golden grid; N1 C = I, K = 2J,
-rectangular C; N3 one-centre closed form, loops, bra-ket symmetry, AO-direct K route.  Nothing is "parity unpinned".
+rectangular C; N3 one-centre closed form, loops, bra-ket symmetry, AO-direct K route; N4 harmonicity, orthogonality and
+norm on the sphere, rotation about z, tabulated low orders, contaminants, adjointness (tests/test_oracle_sph.py).
+Nothing is "parity unpinned".
 
 Nothing here imports the CUDA package except the shared, arithmetic-free input generators.
 """
@@ -378,3 +381,61 @@ def pp_ladder_loops(eri: np.ndarray, C_vir: np.ndarray, X: np.ndarray) -> np.nda
                     for p in range(X.shape[0]):
                         L[p, a, b] += g * X[p, e, f]
     return L
+
+
+# ---------------------------------------------------------------------------------------------------------
+# SURVEY 8(f) N4, second half: the spherical-harmonic transform at matrix level.  The integrals are Cartesian
+# throughout ("730 Cartesian AO"); a caller that works with pure (2l+1) functions converts matrices:
+#     chi^sph_{l m} = sum_c S^l[m, c] chi^cart_c,     c = (a, b, c) lexicographic (reading A7), m = -l..l,
+# with S^l the monomial coefficients of the Racah-normalised real solid harmonic R_lm = r^l sqrt(4 pi/(2l+1)) Y_lm,
+# which has the angular norm of x^l -- the function the caller's N(a,l) normalises (reading A6), so a normalised
+# Cartesian shell gives normalised pure functions.  Written out from the closed form of the real solid harmonics
+# (Helgaker, Jorgensen, Olsen, Molecular Electronic-Structure Theory, Eqs. 6.4.47-6.4.50):
+#     R_lm = N_lm sum_{t=0}^{[(l-|m|)/2]} sum_{u=0}^{t} sum_v C^{lm}_{tuv} x^{2t+|m|-2(u+v)} y^{2(u+v)} z^{l-2t-|m|},
+#     C^{lm}_{tuv} = (-1)^{t+v-v_m} (1/4)^t binom(l,t) binom(l-t,|m|+t) binom(t,u) binom(|m|,2v),
+#     N_lm = 1/(2^{|m|} l!) sqrt(2 (l+|m|)! (l-|m|)! / 2^{delta_{m0}}),
+#     v = v_m, v_m + 1, ..., [|m|/2 - v_m] + v_m,   v_m = 0 (m >= 0), 1/2 (m < 0).
+# Operators (J, K, F) transform as X^sph = S X^cart S^T, densities as D^cart = S^T D^sph S, so that
+# tr(D^sph^T X^sph) = tr(D^cart^T X^cart).
+def sph_matrix(l: int) -> np.ndarray:
+    from math import comb, factorial, sqrt
+    comps = [(i, j, l - i - j) for i in range(l, -1, -1) for j in range(l - i, -1, -1)]
+    S = np.zeros((2 * l + 1, len(comps)))
+    for m in range(-l, l + 1):
+        am = abs(m)
+        N = sqrt(2.0 * factorial(l + am) * factorial(l - am) / (2.0 if m == 0 else 1.0)) / (2.0 ** am * factorial(l))
+        two_vm = 0 if m >= 0 else 1                              # 2 v_m
+        nv = (am - two_vm) // 2                                  # [|m|/2 - v_m]
+        for t in range((l - am) // 2 + 1):
+            for u in range(t + 1):
+                for k in range(nv + 1):                          # v = v_m + k, 2v = 2 v_m + 2k
+                    two_v = two_vm + 2 * k
+                    C = (-1.0) ** (t + k) * 0.25 ** t * comb(l, t) * comb(l - t, am + t) * comb(t, u) * comb(am, two_v)
+                    ex = (2 * t + am - 2 * u - two_v, 2 * u + two_v, l - 2 * t - am)
+                    S[m + l, comps.index(ex)] += N * C
+    return S
+
+
+def sph_block_matrix(b) -> np.ndarray:
+    """S of the whole basis: block diagonal [N_sph, N_cart], shells in the caller's order."""
+    ls = [int(x) for x in np.asarray(b.l)]
+    S = np.zeros((sum(2 * l + 1 for l in ls), sum((l + 1) * (l + 2) // 2 for l in ls)))
+    r = c = 0
+    for l in ls:
+        Sl = sph_matrix(l)
+        S[r:r + Sl.shape[0], c:c + Sl.shape[1]] = Sl
+        r += Sl.shape[0]
+        c += Sl.shape[1]
+    return S
+
+
+def sph_from_cart(b, X: np.ndarray) -> np.ndarray:
+    """Operator matrices [n, N_cart, N_cart] -> [n, N_sph, N_sph]:  S X S^T."""
+    S = sph_block_matrix(b)
+    return np.stack([S @ x @ S.T for x in np.asarray(X, dtype=np.float64)])
+
+
+def cart_from_sph(b, D: np.ndarray) -> np.ndarray:
+    """Density matrices [n, N_sph, N_sph] -> [n, N_cart, N_cart]:  S^T D S."""
+    S = sph_block_matrix(b)
+    return np.stack([S.T @ d @ S for d in np.asarray(D, dtype=np.float64)])
