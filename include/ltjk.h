@@ -33,7 +33,8 @@ extern "C" {
 #define LTJK_EINVAL   -1   /* bad argument (null pointer, negative size, nprim too large, ...) */
 #define LTJK_ENOBASIS -2   /* call order: basis / shell pairs not set yet */
 #define LTJK_ECUDA    -3   /* CUDA runtime error or no device */
-#define LTJK_ELMAX    -4   /* angular momentum > 2 (kernels are Cartesian s, p, d) */
+#define LTJK_ELMAX    -4   /* angular momentum beyond what the called path is built for: l > 3 in ltjk_set_basis (kernels are
+                             Cartesian s, p, d, f); an f shell with pair-list digestion or ltjk_jk_grad */
 #define LTJK_ENOCONV  -5   /* Laplace quadrature did not converge (no silent fallback grid) */
 #define LTJK_ENOMEM   -6   /* device allocation failed */
 
@@ -53,7 +54,9 @@ int ltjk_set_scratch_bytes(ltjk_ctx* ctx, long long bytes);
 /* Basis upload (step a1).  HOST pointers, copied.
  *   xyz[natom*3]        centres, bohr
  *   atom[nshell]        centre index of each shell
- *   l[nshell]           angular momentum, 0..2 (else LTJK_ELMAX)
+ *   l[nshell]           angular momentum, 0..3 (else LTJK_ELMAX).  s, p, d classes run generated straight-line code; every
+ *                       class with an f shell runs the looped kernel (PAPER.md:L316 two codegen regimes).
+ *                       Cartesian components in lexicographic order (f: xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz)
  *   nprim[nshell]       primitives per shell, 1..4
  *   prim_off[nshell]    first primitive of the shell in exps/coef
  *   exps[], coef[]      primitive exponents and coefficients.  coef multiplies
@@ -210,6 +213,11 @@ int ltjk_debug_poison(ltjk_ctx* ctx, int enable);
 /* Test hook: contracted Cartesian shell quartet (A B|C D) in the caller's shell indices, evaluated by the
  * device ERI kernel, written to HOST out[na*nb*nc*nd] (row-major a,b,c,d).  Synchronises. */
 int ltjk_debug_eri_quartet(ltjk_ctx* ctx, int A, int B, int C, int D, double* out_host);
+
+/* Test hook: the same quartet through the LOOPED evaluation (csrc/ltjk_eri_loop.cu) whatever its class.  Classes with an
+ * f shell always take that path; for s, p, d classes this is the cross-check PAPER.md:L316 states for its two codegen
+ * regimes ("machine-epsilon equal to the unrolled path").  Synchronises. */
+int ltjk_debug_eri_quartet_looped(ltjk_ctx* ctx, int A, int B, int C, int D, double* out_host);
 
 /* Test hook: device Boys function F_m(T), m = 0..mmax (mmax <= 8), for n arguments T_host[n];
  * F_host[n*(mmax+1)].  Synchronises. */

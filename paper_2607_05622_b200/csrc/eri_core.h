@@ -25,9 +25,9 @@ constexpr int kPrimStride = 8;        // doubles per primitive pair: p, Px,Py,Pz
 constexpr int kPairHeader = 4;        // ABx, ABy, ABz, npp (as double)
 constexpr int kPairStride = kPairHeader + kMaxPrimPair * kPrimStride;   // doubles per shell pair record
 
-// Boys table: F_m(T_i), T_i = i/8, i = 0..288 (T <= 36), m = 0..16
+// Boys table: F_m(T_i), T_i = i/8, i = 0..288 (T <= 36), m = 0..20
 constexpr int kBoysNT = 289;
-constexpr int kBoysNM = 18;          // orders 0..17: L <= 9 (derivative builds) plus 8 Taylor terms
+constexpr int kBoysNM = 21;          // orders 0..20: L <= 12 ((ff|ff), ltjk_eri_loop.cu) plus 8 Taylor terms
 constexpr double kBoysTmax = 36.0;
 constexpr int kBoysTaylor = 9;        // terms k = 0..8: remainder (1/16)^9/9! ~ 4e-17
 

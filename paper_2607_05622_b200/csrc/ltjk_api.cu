@@ -16,9 +16,9 @@ int set_err(ltjk_ctx* c, int code, const std::string& msg)
     return code;
 }
 
-// Shells per block for l = 0,1,2: 16 / 24 / 24 AOs.  Output blocks of the digestion then have 256, 384 or 576 rows
+// Shells per block for l = 0,1,2,3: 16 / 24 / 24 / 20 AOs.  Output blocks of the digestion then have 256, 384 or 576 rows
 // = 2, 3 or 4.5 row tiles of 128: measured tile fill 94 % against 82 % with the first choice (16/15/18, split evenly).
-static const int kBlkShells[3] = {16, 8, 4};
+static const int kBlkShells[kNumL] = {16, 8, 4, 2};
 static const int kRunMax = 8;                  // panels accumulated in registers before a flush
 
 void free_tables(ltjk_ctx* c)
@@ -57,11 +57,11 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
     auto cls_of = [&](int r) { return pair_class(c->blk_l[c->pair_I[r]], c->blk_l[c->pair_J[r]]); };
     {
         int r = 0;
-        for (int cls = 0; cls < 6; ++cls) {
+        for (int cls = 0; cls < kNumPairCls; ++cls) {
             c->cls_start[cls] = r;
             while (r < npair && cls_of(r) == cls) ++r;
         }
-        c->cls_start[6] = r;
+        c->cls_start[kNumPairCls] = r;
     }
     std::vector<std::vector<int>> byL(nblk);
     Group g;
@@ -120,7 +120,7 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
             if (!open) {
                 g = Group();
                 g.sub0 = (int)c->subs.size(); g.nsub = 0; g.cb = cb; g.nquartets = 0; g.nints = 0.0;
-                for (int k = 0; k < 6; ++k) g.maxkets[k] = 0;
+                for (int k = 0; k < kNumPairCls; ++k) g.maxkets[k] = 0;
                 if (!c->resident) used = 0;             // resident: every group keeps its own region of the panel store
                 open = true;
             }
@@ -133,7 +133,7 @@ void build_work(ltjk_ctx* c, std::vector<DigestItem>& items)
             g.nsub++;
             used += nIJ * (c->koff[r1] - c->koff[r0]);
             g.nints += (double)nIJ * (double)(c->koff[r1] - c->koff[r0]);
-            for (int k = 0; k < 6; ++k) {
+            for (int k = 0; k < kNumPairCls; ++k) {
                 const int a = std::max(r0, c->cls_start[k]), b = std::min(r1, c->cls_start[k + 1]);
                 if (b > a) g.maxkets[k] = std::max(g.maxkets[k], b - a);
             }
@@ -284,7 +284,7 @@ int ltjk_set_basis(ltjk_ctx* c, int natom, const double* xyz, int nshell, const 
     int ntot = 0;
     for (int s = 0; s < nshell; ++s) {
         if (l[s] < 0) return set_err(c, LTJK_EINVAL, "set_basis: negative angular momentum");
-        if (l[s] > 2) return set_err(c, LTJK_ELMAX, "set_basis: angular momentum > 2 (kernels are Cartesian s, p, d)");
+        if (l[s] > 3) return set_err(c, LTJK_ELMAX, "set_basis: angular momentum > 3 (kernels are Cartesian s, p, d, f)");
         if (nprim[s] < 1 || nprim[s] > 4) return set_err(c, LTJK_EINVAL, "set_basis: nprim must be 1..4");
         if (atom[s] < 0 || atom[s] >= natom || prim_off[s] < 0) return set_err(c, LTJK_EINVAL, "set_basis: bad atom/prim_off");
         ntot = std::max(ntot, prim_off[s] + nprim[s]);
@@ -346,7 +346,7 @@ int ltjk_set_basis(ltjk_ctx* c, int natom, const double* xyz, int nshell, const 
     // l-homogeneous blocks of fixed size (the last one of each l takes the remainder)
     c->blk_sh0.clear(); c->blk_nsh.clear(); c->blk_ao0.clear(); c->blk_nao.clear(); c->blk_l.clear();
     int s0 = 0;
-    for (int ll = 0; ll < 3; ++ll) {
+    for (int ll = 0; ll < kNumL; ++ll) {
         int n = 0;
         while (s0 + n < nshell && l[c->sh_int2ext[s0 + n]] == ll) ++n;
         c->max_nsh_l[ll] = 0;

@@ -91,12 +91,16 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     LTJK_CUDA(c, cudaMalloc(&t.schwarz, sizeof(double) * (size_t)ns * ns));
     LTJK_CUDA(c, cudaMemsetAsync(t.schwarz, 0, sizeof(double) * (size_t)ns * ns, c->stream));
     if ((rc = launch_pair_records(c, d_xyz, d_atom, d_l, d_nprim, d_poff, d_exps, d_coef, d_i2e))) return rc;
-    int lrange[4] = {0, 0, 0, ns};
+    int lrange[kNumL + 1] = {0, 0, 0, 0, ns};
+    bool has_f = false;
     for (int s = 0; s < ns; ++s) {
         const int ll = c->l[c->sh_int2ext[s]];
-        if (ll < 1) lrange[1] = s + 1;
-        if (ll < 2) lrange[2] = s + 1;
+        for (int k = 1; k < kNumL; ++k)
+            if (ll < k) lrange[k] = s + 1;
+        has_f = has_f || ll == 3;
     }
+    if (has_f && c->digest_mode_req == 2)
+        return set_err(c, LTJK_ELMAX, "build_shell_pairs: pair-list digestion is built for s, p, d shells; use mode 0 or 1 with f shells");
     if ((rc = launch_schwarz(c, lrange))) return rc;
     c->Qhost.assign((size_t)ns * ns, 0.0);
     LTJK_CUDA(c, cudaMemcpyAsync(c->Qhost.data(), t.schwarz, sizeof(double) * (size_t)ns * ns, cudaMemcpyDeviceToHost,
@@ -128,7 +132,7 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
     {
         const double npairs_all = 0.5 * (double)ns * (ns + 1);
         const double kept_frac = (double)c->n_quartets_kept / (0.5 * npairs_all * (npairs_all + 1.0));
-        c->digest_mode = c->digest_mode_req ? c->digest_mode_req : (kept_frac < 0.5 ? 2 : 1);
+        c->digest_mode = c->digest_mode_req ? c->digest_mode_req : (kept_frac < 0.5 && !has_f ? 2 : 1);
     }
     const bool panels = (c->digest_mode == 1);
     c->subs.clear(); c->groups.clear();
@@ -149,7 +153,7 @@ int ltjk_build_shell_pairs(ltjk_ctx* c, double schwarz_tau, long long* n_pairs, 
             qblk[(size_t)I * nblk + J] = m;
             qmax = std::max(qmax, m);
         }
-    for (int cls = 0; cls < 6; ++cls)
+    for (int cls = 0; cls < kNumPairCls; ++cls)
         for (int I = 0; I < nblk; ++I)
             for (int J = 0; J <= I; ++J)
                 if (pair_class(c->blk_l[I], c->blk_l[J]) == cls && qblk[(size_t)I * nblk + J] * qmax >= schwarz_tau) {
@@ -546,7 +550,7 @@ int ltjk_set_timing(ltjk_ctx* c, int enable)
     return LTJK_OK;
 }
 
-int ltjk_debug_eri_quartet(ltjk_ctx* c, int A, int B, int C, int D, double* out_host)
+static int debug_eri_quartet(ltjk_ctx* c, int A, int B, int C, int D, double* out_host, bool looped)
 {
     if (!c || !out_host) return LTJK_EINVAL;
     if (!c->have_pairs) return set_err(c, LTJK_ENOBASIS, "debug_eri_quartet: shell pairs not built");
@@ -568,7 +572,7 @@ int ltjk_debug_eri_quartet(ltjk_ctx* c, int A, int B, int C, int D, double* out_
     double* d_out = nullptr;
     LTJK_CUDA(c, cudaMalloc(&d_out, sizeof(double) * ntot));
     const int rc = launch_eri_single(c, e2i[sh[pos[0]]], e2i[sh[pos[1]]], e2i[sh[pos[2]]], e2i[sh[pos[3]]], L(0), L(1),
-                                     L(2), L(3), d_out);
+                                     L(2), L(3), d_out, looped);
     if (rc) { cudaFree(d_out); return rc; }
     std::vector<double> tmp(ntot);
     LTJK_CUDA(c, cudaMemcpyAsync(tmp.data(), d_out, sizeof(double) * ntot, cudaMemcpyDeviceToHost, c->stream));
@@ -586,6 +590,16 @@ int ltjk_debug_eri_quartet(ltjk_ctx* c, int A, int B, int C, int D, double* out_
                         tmp[((idx[0] * nc[1] + idx[1]) * nc[2] + idx[2]) * nc[3] + idx[3]];
                 }
     return LTJK_OK;
+}
+
+int ltjk_debug_eri_quartet(ltjk_ctx* c, int A, int B, int C, int D, double* out_host)
+{
+    return debug_eri_quartet(c, A, B, C, D, out_host, false);
+}
+
+int ltjk_debug_eri_quartet_looped(ltjk_ctx* c, int A, int B, int C, int D, double* out_host)
+{
+    return debug_eri_quartet(c, A, B, C, D, out_host, true);
 }
 
 int ltjk_debug_boys(ltjk_ctx* c, int mmax, int n, const double* T_host, double* F_host)

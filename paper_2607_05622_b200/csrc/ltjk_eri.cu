@@ -62,7 +62,7 @@ __global__ void schwarz_kernel(int nshell, int a0, int na, int b0, int nb, const
     Q[(size_t)B * nshell + A] = m;
 }
 
-int launch_schwarz(ltjk_ctx* c, const int* lrange /* host: first internal shell of l = 0,1,2 and end */)
+int launch_schwarz(ltjk_ctx* c, const int* lrange /* host: first internal shell of l = 0,1,2,3 and end */)
 {
     const int ns = c->nshell;
 #define SCHW(LA, LB)                                                                                              \
@@ -76,21 +76,15 @@ int launch_schwarz(ltjk_ctx* c, const int* lrange /* host: first internal shell 
     }
     SCHW(0, 0) SCHW(1, 0) SCHW(1, 1) SCHW(2, 0) SCHW(2, 1) SCHW(2, 2)
 #undef SCHW
+    for (int lb = 0; lb <= 3; ++lb) {                      // pair classes with an f shell: looped kernel
+        const int rc = launch_schwarz_loop(c, 3, lb, lrange[3], lrange[4] - lrange[3], lrange[lb], lrange[lb + 1] - lrange[lb]);
+        if (rc) return rc;
+    }
     return LTJK_OK;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // a6 + a7: panels of one class segment.  Thread -> (ket rank r in [ra,rb), shell quartet inside the block quartet).
-struct EriArgs {
-    DevTables t;
-    const SubChunk* subs;  // sub-chunks of the group; blockIdx.y selects one
-    int ca, cb_;           // rank range [ca, cb_) of the launch's ket pair class
-    int mJ, mK, mL;        // max shells per block of the launch's l_J, l_K, l_L (thread-index decode)
-    int qn;                // mI*mJ*mK*mL
-    double tau;
-    double* panel;         // ring half
-};
-
 template <int LA, int LB, int LC, int LD>
 // (64,4): without a min-blocks hint ptxas drops the heavy classes to 32 registers and spills ~80 KB per thread
 __global__ void __launch_bounds__(64, 4) eri_panel_kernel(const EriArgs g)
@@ -278,7 +272,7 @@ __global__ void __launch_bounds__(kCoopThreads, 1) eri_panel_coop_kernel(const E
     }
 }
 
-static const int kClsLa[6] = {0, 1, 1, 2, 2, 2}, kClsLb[6] = {0, 0, 1, 0, 1, 2};
+static const int kClsLa[kNumPairCls] = {0, 1, 1, 2, 2, 2, 3, 3, 3, 3}, kClsLb[kNumPairCls] = {0, 0, 1, 0, 1, 2, 0, 1, 2, 3};
 
 template <int CB, int CK>
 static int launch_cls(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
@@ -342,6 +336,8 @@ int launch_eri_panels(ltjk_ctx* c, const Group& gr, int ck)
     g.panel = c->d_panel + (size_t)gr.buf * c->panel_half;
     c->st_launches++;
     const int mk = gr.maxkets[ck], ns = gr.nsub;
+    if (cb >= 6)                                            // a class with an f shell (ck <= cb): looped kernel
+        return launch_eri_panels_loop(c, g, kClsLa[cb], kClsLb[cb], kClsLa[ck], kClsLb[ck], mk, ns);
     switch (cb) {
     case 0: return launch_cls_k<0>(c, ck, g, mk, ns);
     case 1: return launch_cls_k<1>(c, ck, g, mk, ns);
@@ -386,11 +382,12 @@ static void single_cls_k(ltjk_ctx* c, int ck, const double* bra, const double* k
 }
 
 // (AB|CD) for INTERNAL shell indices with l_A>=l_B, l_C>=l_D and class(AB) >= class(CD); d_out row-major a,b,c,d.
-int launch_eri_single(ltjk_ctx* c, int A, int B, int C, int D, int la, int lb, int lc, int ld, double* d_out)
+int launch_eri_single(ltjk_ctx* c, int A, int B, int C, int D, int la, int lb, int lc, int ld, double* d_out, bool looped)
 {
     const int cb = la * (la + 1) / 2 + lb, ck = lc * (lc + 1) / 2 + ld;
     const double* bra = c->t.pair_rec + ((size_t)A * c->nshell + B) * c->t.rec_stride;
     const double* ket = c->t.pair_rec + ((size_t)C * c->nshell + D) * c->t.rec_stride;
+    if (cb >= 6 || looped) return launch_eri_single_loop(c, bra, ket, la, lb, lc, ld, d_out);
     switch (cb) {
     case 0: single_cls_k<0>(c, ck, bra, ket, d_out); break;
     case 1: single_cls_k<1>(c, ck, bra, ket, d_out); break;

@@ -269,6 +269,8 @@ extern "C" int ltjk_jk_grad(ltjk_ctx* c, int nP, const double* A, const double* 
     if (!c) return LTJK_EINVAL;
     if (!c->have_basis) return set_err(c, LTJK_ENOBASIS, "jk_grad: no basis");
     if (nP <= 0 || !A || !B || (!gradJ && !gradK)) return set_err(c, LTJK_EINVAL, "jk_grad: bad arguments");
+    for (int l : c->l)
+        if (l > 2) return set_err(c, LTJK_ELMAX, "jk_grad: the derivative classes are generated for s, p, d shells (an f shell would need g)");
     cudaSetDevice(c->device);
     return launch_jk_grad(c, nP, A, B, gradJ, gradK);
 }

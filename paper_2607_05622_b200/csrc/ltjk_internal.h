@@ -8,6 +8,8 @@
 
 namespace ltjk {
 
+constexpr int kNumL = 4;           // angular momenta s, p, d, f (f: SURVEY.md 8(f) N4, looped ERI kernel ltjk_eri_loop.cu)
+constexpr int kNumPairCls = kNumL * (kNumL + 1) / 2;   // block-pair classes (la >= lb), la(la+1)/2 + lb
 constexpr int kDigestRows = 128;   // output rows per digestion CTA (ltjk_digest.cu) = row-tile height of the work items
 
 // ---- geometry-frozen device tables (built by ltjk_build_shell_pairs, reused by every jk_build) ----------------
@@ -65,7 +67,7 @@ struct Group {
     int buf;                // ring half
     long long item0;        // first digest item: nitemsJ J-view items, then nitemsK K-view items
     int nitemsJ, nitemsK;
-    int maxkets[6];         // per ket class: max number of kets of that class in one sub-chunk
+    int maxkets[kNumPairCls]; // per ket class: max number of kets of that class in one sub-chunk
     long long nquartets;    // shell quartets evaluated
     double nints;           // integrals in the panels
 };
@@ -150,8 +152,8 @@ struct ltjk_ctx {
     std::vector<double> Qhost;            // internal order [nshell*nshell]
     std::vector<ltjk::SubChunk> subs;
     std::vector<ltjk::Group> groups;
-    int cls_start[7] = {0, 0, 0, 0, 0, 0, 0};   // first rank of each pair class
-    int max_nsh_l[3] = {0, 0, 0};         // max shells per block for each l
+    int cls_start[ltjk::kNumPairCls + 1] = {};          // first rank of each pair class
+    int max_nsh_l[ltjk::kNumL] = {};            // max shells per block for each l
     double tau = 0.0;
     long long n_quartets_kept = 0;
 
@@ -229,9 +231,24 @@ void digest_colblocks(int nD, int mode, int* TN, int* ncolblk);
 // ltjk_eri.cu
 int launch_pair_records(ltjk_ctx* c, const double* d_xyz, const int* d_atom, const int* d_l, const int* d_nprim,
                         const int* d_poff, const double* d_exps, const double* d_coef, const int* d_int2ext);
+// arguments of the panel-writing ERI kernels (ltjk_eri.cu, ltjk_eri_loop.cu)
+struct EriArgs {
+    DevTables t;
+    const SubChunk* subs;  // sub-chunks of the group; blockIdx.y selects one
+    int ca, cb_;           // rank range [ca, cb_) of the launch's ket pair class
+    int mJ, mK, mL;        // max shells per block of the launch's l_J, l_K, l_L (thread-index decode)
+    int qn;                // mI*mJ*mK*mL
+    double tau;
+    double* panel;         // ring half
+};
+
 int launch_schwarz(ltjk_ctx* c, const int* lrange_host);
 int launch_eri_panels(ltjk_ctx* c, const Group& g, int ck);
-int launch_eri_single(ltjk_ctx* c, int A, int B, int C, int D, int la, int lb, int lc, int ld, double* d_out);
+int launch_eri_single(ltjk_ctx* c, int A, int B, int C, int D, int la, int lb, int lc, int ld, double* d_out, bool looped);
+// ltjk_eri_loop.cu: classes with an f shell (looped evaluation, one CTA per contracted quartet)
+int launch_eri_panels_loop(ltjk_ctx* c, const EriArgs& g, int la, int lb, int lc, int ld, int maxkets, int nsub);
+int launch_eri_single_loop(ltjk_ctx* c, const double* bra, const double* ket, int la, int lb, int lc, int ld, double* d_out);
+int launch_schwarz_loop(ltjk_ctx* c, int la, int lb, int a0, int na, int b0, int nb);
 int launch_boys_debug(ltjk_ctx* c, int mmax, int n, const double* d_T, double* d_F);
 
 // ltjk_pair.cu, ltjk_peri.cu, ltjk_pdigest.cu: pair-list formulation

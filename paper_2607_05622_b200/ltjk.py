@@ -23,7 +23,7 @@ ERRORS = {0: "LTJK_OK", -1: "LTJK_EINVAL", -2: "LTJK_ENOBASIS", -3: "LTJK_ECUDA"
 EXPORTS = [
     "ltjk_create", "ltjk_destroy", "ltjk_last_error", "ltjk_set_scratch_bytes", "ltjk_set_basis", "ltjk_get_nao",
     "ltjk_build_shell_pairs", "ltjk_get_schwarz", "ltjk_laplace_quadrature", "ltjk_build_pseudo_densities", "ltjk_build_pseudo_densities_noalloc",
-    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_laplace_fock", "ltjk_laplace_accumulate", "ltjk_pp_ladder", "ltjk_jk_grad", "ltjk_get_stats", "ltjk_set_timing", "ltjk_set_digest_mode", "ltjk_get_digest_mode", "ltjk_set_resident", "ltjk_set_quartet_shard", "ltjk_debug_poison", "ltjk_debug_eri_quartet",
+    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_laplace_fock", "ltjk_laplace_accumulate", "ltjk_pp_ladder", "ltjk_jk_grad", "ltjk_get_stats", "ltjk_set_timing", "ltjk_set_digest_mode", "ltjk_get_digest_mode", "ltjk_set_resident", "ltjk_set_quartet_shard", "ltjk_debug_poison", "ltjk_debug_eri_quartet", "ltjk_debug_eri_quartet_looped",
     "ltjk_debug_boys", "ltjk_bench_dfma_peak", "ltjk_bench_copy_peak",
 ]
 
@@ -263,12 +263,12 @@ class Context:
     def set_timing(self, enable: bool):
         self._chk(self.lib.ltjk_set_timing(self._h, ctypes.c_int(1 if enable else 0)))
 
-    def debug_eri_quartet(self, basis, A, B, C, D) -> np.ndarray:
-        nc = (1, 3, 6)
+    def debug_eri_quartet(self, basis, A, B, C, D, looped: bool = False) -> np.ndarray:
+        nc = (1, 3, 6, 10)
         shp = tuple(nc[int(basis.l[s])] for s in (A, B, C, D))
         out = np.zeros(shp)
-        self._chk(self.lib.ltjk_debug_eri_quartet(self._h, ctypes.c_int(A), ctypes.c_int(B), ctypes.c_int(C),
-                                                  ctypes.c_int(D), _d(out)))
+        fn = self.lib.ltjk_debug_eri_quartet_looped if looped else self.lib.ltjk_debug_eri_quartet
+        self._chk(fn(self._h, ctypes.c_int(A), ctypes.c_int(B), ctypes.c_int(C), ctypes.c_int(D), _d(out)))
         return out
 
     def debug_boys(self, mmax: int, T) -> np.ndarray:

@@ -1,0 +1,135 @@
+"""GPU parity for SURVEY.md 8(f) row N4, f shells (the looped codegen regime): every class with an f
+shell goes through csrc/ltjk_eri_loop.cu.  The oracle side is pinned at l = 3 by tests/test_oracle_eri.py (198-digit
+centre derivatives of the closed-form (ss|ss) up to (ff|ff))."""
+import itertools
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2607_05622_b200.inputs import custom_basis, random_densities
+from test_gpu_parity import TOL, gpu_jk, make_ctx, relerr, torch_cuda  # noqa: F401  (fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+def four_centre_basis(lmax):
+    rng = np.random.default_rng(7)
+    xyz = rng.uniform(-1.5, 1.5, size=(4, 3))
+    xyz[3] = xyz[0]                                              # two coincident centres
+    shells = []
+    for ia in range(4):
+        shells.append([(l, [0.3 + 0.4 * ia + 0.2 * l, 1.1 + 0.3 * ia + 0.5 * l], [0.6, 0.4]) for l in range(lmax + 1)])
+    return custom_basis(xyz, shells)
+
+
+def test_eri_f_classes_vs_oracle(torch_cuda):
+    """All 175 ordered classes (la lb|lc ld), l <= 3, with at least one f shell, two-primitive contractions: the
+    looped kernel against the oracle."""
+    b = four_centre_basis(3)
+    ctx = make_ctx(b)
+    worst = 0.0
+    for ls in itertools.product(range(4), repeat=4):
+        if 3 not in ls:
+            continue
+        A, B, C, D = (4 * i + l for i, l in enumerate(ls))
+        out = ctx.debug_eri_quartet(b, A, B, C, D)
+        ref = O.eri_shell(b, A, B, C, D)
+        err = np.abs(out - ref).max() / np.abs(ref).max()
+        worst = max(worst, err)
+        assert err < 1e-12, (ls, err)
+    assert worst < 1e-12
+
+
+def test_looped_path_equals_unrolled_path_spd(torch_cuda):
+    """the looped regime is "machine-epsilon equal to the unrolled path": all 81 s/p/d classes through
+    both of the library's evaluations (generated OS/HGP straight-line code vs the looped Hermite kernel)."""
+    b = four_centre_basis(2)
+    ctx = make_ctx(b)
+    for ls in itertools.product(range(3), repeat=4):
+        A, B, C, D = (3 * i + l for i, l in enumerate(ls))
+        u = ctx.debug_eri_quartet(b, A, B, C, D)
+        v = ctx.debug_eri_quartet(b, A, B, C, D, looped=True)
+        assert np.abs(u - v).max() <= 2e-13 * np.abs(u).max(), ls
+
+
+def spdf_basis(natom=3, seed=5):
+    rng = np.random.default_rng(seed)
+    xyz = rng.uniform(-2.0, 2.0, size=(natom, 3))
+    shells = []
+    for ia in range(natom):
+        sh = [(0, [2.1 + ia, 0.5], [0.5, 0.6]), (0, [0.25 + 0.05 * ia], [1.0]), (1, [0.9 + 0.1 * ia, 0.3], [0.4, 0.7]),
+              (2, [0.8 + 0.1 * ia], [1.0]), (3, [0.7 + 0.15 * ia], [1.0])]
+        if ia == 0:
+            sh.append((3, [1.3, 0.45], [0.55, 0.5]))              # a contracted f shell, a second f on one centre
+            sh.append((3, [0.35], [1.0]))                        # three f shells: a full block of two plus a remainder
+        shells.append(sh)
+    return custom_basis(xyz, shells)
+
+
+def test_schwarz_f_vs_oracle(torch_cuda):
+    b = spdf_basis()
+    ctx = make_ctx(b)
+    Q = ctx.get_schwarz()
+    Qr = O.schwarz(b)
+    assert np.abs(Q ** 2 - Qr ** 2).max() <= 1e-13 * np.abs(Qr ** 2).max()
+    big = Qr > 1e-4
+    assert np.abs(Q[big] / Qr[big] - 1.0).max() <= 1e-10
+
+
+@pytest.mark.parametrize("scratch", [None, 1 << 20])
+def test_jk_spdf_vs_definition(torch_cuda, scratch):
+    """s, p, d and f shells (all 55 canonical classes, diagonal f blocks, an f remainder block) against Eq. 17 literally
+    (oracle O7 tensor, no symmetry): non-symmetric densities, nothing screened.  The 1 MiB ring splits the build into
+    many launch units."""
+    b = spdf_basis()
+    D = random_densities(b.nao, 5, seed=21)
+    ctx = make_ctx(b, tau=0.0, scratch=scratch)
+    assert ctx.get_digest_mode() == 1                           # f shells: block panels
+    J, K = gpu_jk(torch_cuda, ctx, D)
+    Jr, Kr = O.jk_definition(O.eri_tensor(b), D)
+    assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
+    assert np.abs(K - K.transpose(0, 2, 1)).max() > 1e-3 * np.abs(K).max()
+
+
+def test_jk_spdf_screened_vs_folded(torch_cuda):
+    """An extended chain with f shells and the production threshold: GPU vs the oracle's canonical-quartet digestion O6
+    with the same Schwarz predicate."""
+    rng = np.random.default_rng(31)
+    natom = 8
+    xyz = np.stack([3.2 * np.arange(natom), 0.4 * rng.standard_normal(natom), 0.4 * rng.standard_normal(natom)], 1)
+    shells = [[(0, [1.9, 0.45], [0.5, 0.6]), (1, [0.8], [1.0]), (2, [0.7], [1.0]), (3, [0.9 + 0.05 * ia], [1.0])]
+              for ia in range(natom)]
+    b = custom_basis(xyz, shells)
+    D = random_densities(b.nao, 18, seed=22)                     # 18 densities: two column blocks, a ragged one
+    ctx = make_ctx(b, tau=1e-10)
+    J, K = gpu_jk(torch_cuda, ctx, D)
+    Jr, Kr, kept = O.jk_folded(b, D, 1e-10)
+    npair = b.nshell * (b.nshell + 1) // 2
+    assert 0 < kept < npair * (npair + 1) // 2                   # the threshold really drops quartets here
+    assert relerr(J, Jr) < TOL and relerr(K, Kr) < TOL
+
+
+def test_f_shell_limits(torch_cuda):
+    """What is not built for f shells fails loudly: pair-list digestion, derivative builds, l = 4."""
+    from paper_2607_05622_b200 import ltjk
+    from paper_2607_05622_b200.inputs import Basis
+    b = spdf_basis(natom=2)
+    ctx = ltjk.Context(0)
+    ctx.set_digest_mode(2)
+    ctx.set_basis(b)
+    with pytest.raises(ltjk.LtjkError) as e:
+        ctx.build_shell_pairs(1e-12)
+    assert e.value.code == -4
+    ctx.set_digest_mode(0)
+    ctx.build_shell_pairs(1e-12)
+    A = torch_cuda.zeros((1, b.nao, b.nao), dtype=torch_cuda.float64, device="cuda")
+    g = torch_cuda.zeros((1, 2, 3), dtype=torch_cuda.float64, device="cuda")
+    with pytest.raises(ltjk.LtjkError) as e:
+        ctx.jk_grad(A, A, g, g.clone())
+    assert e.value.code == -4
+    bad = Basis(np.zeros((1, 3)), np.zeros(1, np.int32), np.array([4], np.int32), np.ones(1, np.int32),
+                np.zeros(1, np.int32), np.ones(1), np.ones(1), np.array([0, 15]))   # a g shell
+    with pytest.raises(ltjk.LtjkError) as e:
+        ctx.set_basis(bad)
+    assert e.value.code == -4

@@ -292,7 +292,7 @@ def test_full_size_large_subset_closure(torch_cuda):
 
 
 def test_edge_cases_and_error_codes(torch_cuda, tiny):
-    """Degenerate inputs through the C ABI: call-order errors, l > 2, bad sizes, one density, a density count that
+    """Degenerate inputs through the C ABI: call-order errors, l > 3, bad sizes, one density, a density count that
     needs several column blocks (nD = 200 > 192), a one-shell basis (a single, fully diagonal block quartet)."""
     torch = torch_cuda
     from paper_2607_05622_b200 import ltjk
@@ -302,8 +302,8 @@ def test_edge_cases_and_error_codes(torch_cuda, tiny):
         ctx.jk_build(D1, torch.empty_like(D1), torch.empty_like(D1))
     assert e.value.code == -2                                     # LTJK_ENOBASIS
     from paper_2607_05622_b200.inputs import Basis
-    bad = Basis(np.zeros((1, 3)), np.zeros(1, np.int32), np.array([3], np.int32), np.ones(1, np.int32),
-                np.zeros(1, np.int32), np.ones(1), np.ones(1), np.array([0, 10]))   # an f shell
+    bad = Basis(np.zeros((1, 3)), np.zeros(1, np.int32), np.array([4], np.int32), np.ones(1, np.int32),
+                np.zeros(1, np.int32), np.ones(1), np.ones(1), np.array([0, 15]))   # a g shell
     with pytest.raises(ltjk.LtjkError) as e:
         ctx.set_basis(bad)
     assert e.value.code == -4                                     # LTJK_ELMAX
