@@ -35,7 +35,7 @@ def metric_name(w):
 def kept_integrals(Q, l, tau):
     """Unique (8-fold folded) Cartesian integrals the folded loop digests: sum over canonical shell quartets
     (AB)>=(CD) with Q_AB Q_CD >= tau of na nb nc nd  (oracle O6 / SURVEY 8.0 `ints`)."""
-    nc = np.array([1, 3, 6])[np.asarray(l)]
+    nc = np.array([1, 3, 6, 10])[np.asarray(l)]
     ns = len(l)
     iu = np.tril_indices(ns)
     q = Q[iu]
@@ -87,7 +87,7 @@ class ClockSampler:
 def pair_integrals(Q, l, tau):
     """Per bra shell pair p (canonical order A(A+1)/2+B of the folded loop O6): number of kept unique integrals of its
     quartets (p | q <= p).  Pure counting from the Schwarz bounds; used to scale oracle samples."""
-    nc = np.array([1, 3, 6])[np.asarray(l)]
+    nc = np.array([1, 3, 6, 10])[np.asarray(l)]
     ns = len(l)
     iu = np.tril_indices(ns)
     qv = Q[iu]
@@ -503,6 +503,34 @@ def main():
                                      "(M, N, {K,R}), derivative integrals contracted on the fly"}
         launches += c3.get_stats()["n_launches"]
         c3.close()
+    if world == 1 and not args.no_large:
+        # f shells (looped ERI kernel) -- the medium geometry with an f shell on every heavy atom, one
+        # sweep of its 80 pseudo-densities; then the matrix-level spherical transform of the 80 J matrices
+        wf = make_workload("medium_f")
+        repf = sweep_report(torch, ltjk, wf, local, wf.T, 2, 1, 1, barrier, max_over_ranks, want_e2e=False, mode=0)
+        rf, intsf = roofline_of(torch, repf["ctx"], wf, repf, peak_tf)
+        cf = repf["ctx"]
+        nsph = cf.get_nsph()
+        Js = torch.empty((wf.nD, nsph, nsph), dtype=torch.float64, device="cuda")
+        cf.sph_from_cart(repf["J"], Js)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(10):
+            cf.sph_from_cart(repf["J"], Js)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t_sph = e0.elapsed_time(e1) / 10
+        gbs = 8e-9 * wf.nD * (wf.nao ** 2 + nsph ** 2) / (t_sph * 1e-3)
+        config["f_shells_medium_f"] = {
+            "workload": "medium geometry, heavy atoms 4s3p1d1f (400 Cartesian AO, 10 f shells), %d densities" % wf.nD,
+            "value": wf.nD / (repf["ms_per_step"] * 1e-3), "unit": UNIT, "ms_per_step": repf["ms_per_step"], "steps": 2,
+            "warmup": 1, "unique_integrals_kept": intsf, "eri_ms_per_sweep": rf["eri_ms_per_sweep"],
+            "digest_ms_per_sweep": rf["digest_ms_per_sweep"], "digest_frac_of_dfma_peak": rf["frac"],
+            "sph_from_cart": {"n_sph": nsph, "ms": t_sph, "gbs": gbs, "frac_of_hbm_peak": gbs / hbm_peak,
+                              "bytes": "8 (N^2 + N_sph^2) per matrix"},
+            "note": "classes with an f shell run the looped kernel (csrc/ltjk_eri_loop.cu, one CTA per quartet)"}
+        launches += int(repf["launches_per_step"] * 3) + 11
+        cf.close()
     if world == 1 and not args.no_large and w.name != "large":
         wl = make_workload("large")
         s2 = ClockSampler(local)

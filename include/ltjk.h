@@ -146,6 +146,21 @@ int ltjk_laplace_fock(ltjk_ctx* ctx, int nD, const double* J, const double* K, i
 int ltjk_laplace_accumulate(ltjk_ctx* ctx, int ntau, int nT, long long nelem, const double* tau_host,
                             const double* w_host, double omega, const double* X, double* Y);
 
+/* SURVEY 8(f) N4 (second half): spherical-harmonic transform at matrix level.  The integral path is Cartesian
+ * (PAPER.md:L565 counts Cartesian AOs); a caller that works with pure functions converts matrices on the device.
+ * Pure functions of a shell: chi^sph_{l m} = sum_c S^l[m][c] chi^cart_c, m = -l..l in this order, S^l the monomial
+ * coefficients of the Racah-normalised real solid harmonic r^l sqrt(4 pi/(2l+1)) Y_lm (cos(m phi) for m > 0,
+ * sin(|m| phi) for m < 0, positive leading coefficient; p = (y, z, x)): a shell whose x^l component is normalised
+ * (reading A6) gives normalised pure functions.  Shell order and AO order are the caller's.
+ *   ltjk_get_nsph       N_sph = sum over shells of (2l+1)
+ *   ltjk_sph_from_cart  operators (J, K, F):  X_sph = S X_cart S^T,  [nmat][N][N] -> [nmat][N_sph][N_sph]
+ *   ltjk_cart_from_sph  densities:            D_cart = S^T D_sph S,  [nmat][N_sph][N_sph] -> [nmat][N][N]
+ * so that tr(D_sph^T X_sph) = tr(D_cart^T X_cart).  DEVICE pointers, row-major, 1 <= nmat <= 65535, outputs
+ * overwritten, input and output must not overlap; work is enqueued on the ctx stream. */
+int ltjk_get_nsph(const ltjk_ctx* ctx, int* nsph);
+int ltjk_sph_from_cart(ltjk_ctx* ctx, int nmat, const double* X_cart, double* X_sph);
+int ltjk_cart_from_sph(ltjk_ctx* ctx, int nmat, const double* D_sph, double* D_cart);
+
 /* AO-direct particle-particle ladder (Algorithm 2; L432-434)
  *     L[p][a][b] = sum_{e,f} (ae|bf) X[p][e][f],      p = 0..npair-1 a compound occupied-pair index (ij),
  * with (ae|bf) the integrals over the virtual orbitals C_vir [N][nvir], never formed: every X_p is turned into the

@@ -21,7 +21,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 CU_SOURCES = ["ltjk_api.cu", "ltjk_build.cu", "ltjk_eri.cu", "ltjk_digest.cu", "ltjk_transform.cu", "ltjk_pair.cu",
-              "ltjk_peri.cu", "ltjk_pdigest.cu", "ltjk_grad.cu", "ltjk_eri_loop.cu"]
+              "ltjk_peri.cu", "ltjk_pdigest.cu", "ltjk_grad.cu", "ltjk_eri_loop.cu", "ltjk_sph.cu"]
 CPP_SOURCES = ["ltjk_laplace.cpp"]
 HEADERS = ["ltjk_internal.h", "digest_common.h", "eri_core.h", "boys_table.h", "../../include/ltjk.h", "gen_eri.py"]
 

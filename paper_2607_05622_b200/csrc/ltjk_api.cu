@@ -257,6 +257,7 @@ int ltjk_destroy(ltjk_ctx* c)
     free_tables(c);
     free_work(c);
     free_grad(c);
+    free_sph(c);
     if (c->t.boys) cudaFree(c->t.boys);
     for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_eri[i]); cudaEventDestroy(c->ev_dig[i]); }
     cudaEventDestroy(c->ev_start);
@@ -294,6 +295,7 @@ int ltjk_set_basis(ltjk_ctx* c, int natom, const double* xyz, int nshell, const 
     cudaSetDevice(c->device);
     free_tables(c);
     free_grad(c);
+    free_sph(c);
     c->natom = natom; c->nshell = nshell;
     c->xyz.assign(xyz, xyz + 3 * natom);
     c->atom.assign(atom, atom + nshell); c->l.assign(l, l + nshell);

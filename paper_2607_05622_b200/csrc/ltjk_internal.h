@@ -188,6 +188,7 @@ struct ltjk_ctx {
     double *gr_xyz = nullptr, *gr_exps = nullptr, *gr_coef = nullptr;   // basis in caller order for ltjk_jk_grad (ltjk_grad.cu)
     int* gr_int = nullptr;
     int gr_cnt[3] = {0, 0, 0};
+    int* d_sph_meta = nullptr;            // ltjk_sph.cu: shell tables in the caller's order (built on first use)
     bool debug_poison = false;             // test hook: the staging ring is filled with NaN before every chunk / group
     int cur_nD = 0;                        // density count of the build in progress (un-padded)
     int shard_rank = 0, shard_world = 1;   // quartet-space split of one build over ranks (ltjk_set_quartet_shard)
@@ -273,6 +274,8 @@ int launch_pseudo_densities(ltjk_ctx* c, int nocc, int nvir, const double* C_occ
 
 // ltjk_grad.cu
 void free_grad(ltjk_ctx* c);
+// ltjk_sph.cu
+void free_sph(ltjk_ctx* c);
 int launch_jk_grad(ltjk_ctx* c, int nP, const double* A, const double* B, double* gJ, double* gK);
 
 int noalloc_setup(ltjk_ctx* c);            // resolves the static scratch of the no-allocation entry point (set-up)

@@ -64,6 +64,8 @@ ATOM_TYPES = {
     "H2": _even_tempered_contracted(4, 3, 2),  # 25 AO
     "M": _even_tempered_contracted(3, 2, 1),  # 15 AO
     "L": _even_tempered_contracted(2, 1, 0),  # 5 AO
+    # the heavy-atom set plus one uncontracted f polarisation shell (triple-zeta-class bases): 29 AO
+    "HF": _even_tempered_contracted(4, 3, 1) + [(3, [0.9], [1.0])],
 }
 
 
@@ -246,15 +248,19 @@ class Workload:
 
 
 def make_workload(name: str) -> Workload:
-    """Build the seeded workload for one of CONFIG_NAMES."""
-    ci = CONFIG_NAMES.index(name)
+    """Build the seeded workload for one of CONFIG_NAMES, or "<name>_f": the same geometry, sizes and seeds with an
+    f shell added to every heavy atom (type H -> HF; "medium_f" = 400 AO, 10 f shells)."""
+    base = name[:-2] if name.endswith("_f") else name
+    ci = CONFIG_NAMES.index(base)
     rng = np.random.default_rng(SEED0 + ci)
-    xyz = _geometry(name, rng)
-    types = _atom_types(name, rng)
+    xyz = _geometry(base, rng)
+    types = _atom_types(base, rng)
+    if name != base:
+        types = ["HF" if t == "H" else t for t in types]
     basis = make_basis(xyz, types)
     n = basis.nao
-    assert n == _EXPECTED_NAO[name], (name, n)
-    nocc, ntau, nT = _PARAMS[name]
+    assert n == _EXPECTED_NAO[base] + 10 * types.count("HF"), (name, n)
+    nocc, ntau, nT = _PARAMS[base]
     nvir = n - nocc
     C = rng.standard_normal((n, n)) / math.sqrt(n)
     eps_occ = np.sort(rng.uniform(-1.5, -0.3, size=nocc))

@@ -23,7 +23,7 @@ ERRORS = {0: "LTJK_OK", -1: "LTJK_EINVAL", -2: "LTJK_ENOBASIS", -3: "LTJK_ECUDA"
 EXPORTS = [
     "ltjk_create", "ltjk_destroy", "ltjk_last_error", "ltjk_set_scratch_bytes", "ltjk_set_basis", "ltjk_get_nao",
     "ltjk_build_shell_pairs", "ltjk_get_schwarz", "ltjk_laplace_quadrature", "ltjk_build_pseudo_densities", "ltjk_build_pseudo_densities_noalloc",
-    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_laplace_fock", "ltjk_laplace_accumulate", "ltjk_pp_ladder", "ltjk_jk_grad", "ltjk_get_stats", "ltjk_set_timing", "ltjk_set_digest_mode", "ltjk_get_digest_mode", "ltjk_set_resident", "ltjk_set_quartet_shard", "ltjk_debug_poison", "ltjk_debug_eri_quartet", "ltjk_debug_eri_quartet_looped",
+    "ltjk_jk_build", "ltjk_jk_build_host", "ltjk_sweep_host", "ltjk_laplace_fock", "ltjk_laplace_accumulate", "ltjk_pp_ladder", "ltjk_jk_grad", "ltjk_get_nsph", "ltjk_sph_from_cart", "ltjk_cart_from_sph", "ltjk_get_stats", "ltjk_set_timing", "ltjk_set_digest_mode", "ltjk_get_digest_mode", "ltjk_set_resident", "ltjk_set_quartet_shard", "ltjk_debug_poison", "ltjk_debug_eri_quartet", "ltjk_debug_eri_quartet_looped",
     "ltjk_debug_boys", "ltjk_bench_dfma_peak", "ltjk_bench_copy_peak",
 ]
 
@@ -225,6 +225,19 @@ class Context:
         """ltjk_pp_ladder: L[p] = C_vir^T K[C_vir X[p] C_vir^T] C_vir = sum_ef (ae|bf) X[p,e,f]; device tensors."""
         self._chk(self.lib.ltjk_pp_ladder(self._h, ctypes.c_int(C_vir.shape[1]), _devptr(C_vir),
                                           ctypes.c_int(X.shape[0]), _devptr(X), _devptr(L), ctypes.c_int(int(chunk))))
+
+    def get_nsph(self) -> int:
+        n = ctypes.c_int(0)
+        self._chk(self.lib.ltjk_get_nsph(self._h, ctypes.byref(n)))
+        return n.value
+
+    def sph_from_cart(self, X_cart, X_sph):
+        """ltjk_sph_from_cart: operators [nmat,N,N] -> [nmat,N_sph,N_sph] (device tensors), S X S^T."""
+        self._chk(self.lib.ltjk_sph_from_cart(self._h, ctypes.c_int(X_cart.shape[0]), _devptr(X_cart), _devptr(X_sph)))
+
+    def cart_from_sph(self, D_sph, D_cart):
+        """ltjk_cart_from_sph: densities [nmat,N_sph,N_sph] -> [nmat,N,N] (device tensors), S^T D S."""
+        self._chk(self.lib.ltjk_cart_from_sph(self._h, ctypes.c_int(D_sph.shape[0]), _devptr(D_sph), _devptr(D_cart)))
 
     def jk_grad(self, A, B, gradJ, gradK):
         """ltjk_jk_grad: J^x(A,B), K^x(A,B) (Eq. 18) for device tensors A, B [nP,N,N] -> gradJ, gradK [nP,natom,3]."""

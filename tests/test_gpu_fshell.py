@@ -133,3 +133,45 @@ def test_f_shell_limits(torch_cuda):
     with pytest.raises(ltjk.LtjkError) as e:
         ctx.set_basis(bad)
     assert e.value.code == -4
+
+
+def test_sph_transform_vs_oracle(torch_cuda):
+    """Matrix-level spherical transform, both directions, s/p/d/f shells interleaved in the caller's order, against the
+    oracle's S X S^T / S^T D S (plain matmuls with the closed-form solid harmonics)."""
+    torch = torch_cuda
+    b = spdf_basis()
+    ctx = make_ctx(b)
+    ns = ctx.get_nsph()
+    assert ns == int(sum(2 * l + 1 for l in b.l)) and ns < b.nao
+    rng = np.random.default_rng(41)
+    X = rng.standard_normal((3, b.nao, b.nao))
+    D = rng.standard_normal((3, ns, ns))
+    Xs = torch.empty((3, ns, ns), dtype=torch.float64, device="cuda")
+    Dc = torch.empty((3, b.nao, b.nao), dtype=torch.float64, device="cuda")
+    ctx.sph_from_cart(torch.from_numpy(X).cuda(), Xs)
+    ctx.cart_from_sph(torch.from_numpy(D).cuda(), Dc)
+    torch.cuda.synchronize()
+    assert relerr(Xs.cpu().numpy(), O.sph_from_cart(b, X)) < 1e-13
+    assert relerr(Dc.cpu().numpy(), O.cart_from_sph(b, D)) < 1e-13
+
+
+def test_jk_in_the_pure_basis_end_to_end(torch_cuda):
+    """J and K of non-symmetric densities given in the PURE basis: cart_from_sph -> jk_build -> sph_from_cart on the
+    device, against the oracle's composition (O7 tensor, Eq. 17, the oracle's own transforms)."""
+    torch = torch_cuda
+    b = spdf_basis()
+    ctx = make_ctx(b, tau=0.0)
+    ns = ctx.get_nsph()
+    Ds = np.random.default_rng(42).standard_normal((4, ns, ns))
+    Dc = torch.empty((4, b.nao, b.nao), dtype=torch.float64, device="cuda")
+    ctx.cart_from_sph(torch.from_numpy(Ds).cuda(), Dc)
+    J, K = torch.empty_like(Dc), torch.empty_like(Dc)
+    ctx.jk_build(Dc, J, K)
+    Js = torch.empty((4, ns, ns), dtype=torch.float64, device="cuda")
+    Ks = torch.empty_like(Js)
+    ctx.sph_from_cart(J, Js)
+    ctx.sph_from_cart(K, Ks)
+    torch.cuda.synchronize()
+    Jr, Kr = O.jk_definition(O.eri_tensor(b), O.cart_from_sph(b, Ds))
+    assert relerr(Js.cpu().numpy(), O.sph_from_cart(b, Jr)) < TOL
+    assert relerr(Ks.cpu().numpy(), O.sph_from_cart(b, Kr)) < TOL
