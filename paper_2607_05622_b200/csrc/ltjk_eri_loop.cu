@@ -5,8 +5,8 @@
 // code of csrc/gen/ stops at (dd|dd); every class with an l = 3 shell comes here.  Angular momenta are run-time
 // arguments, the recurrences are loops over small index tables built in shared memory, and -- unlike the paper's
 // one-thread-per-quartet mapping, whose per-thread working set ((ff|ff): 10^4 outputs) only fits an HBM scratch slab
-// -- one 64-thread CTA evaluates one contracted shell quartet with the whole working set in shared memory
-// ((ff|ff): 84 KB, two CTAs per SM).  The evaluation is the Hermite route (Gaussian product -> Hermite expansion
+// -- one warp (a 32-thread CTA) evaluates one contracted shell quartet with the whole working set in shared memory
+// ((ff|ff): 84 KB, two quartets per SM; the classes with one f shell: 2-15 KB, 16 quartets per SM).  The evaluation is the Hermite route (Gaussian product -> Hermite expansion
 // coefficients E, Hermite Coulomb integrals R from the Boys function, two short box sums), which needs no horizontal
 // stage and whose loops have fixed, table-free trip counts; DESIGN.md section 4c states the difference from the
 // paper's looped HGP-OS and the measured cost.
@@ -21,7 +21,8 @@
 
 namespace ltjk {
 
-constexpr int kLoopThreads = 64;
+constexpr int kLoopThreads = 32;      // one warp per quartet: every barrier below is a __syncwarp
+constexpr int kLoopMinBlocks = 32;    // register cap 64: the kernel is latency-bound, resident quartets per SM matter most
 
 __host__ __device__ inline int tet(int L) { return (L + 1) * (L + 2) * (L + 3) / 6; }   // #{(t,u,v): t+u+v <= L}
 
@@ -89,14 +90,13 @@ __device__ void hermite_table(const int la, const int lb, const double p, const 
 {
     const int nt = la + lb + 1, sj = nt, si = (lb + 1) * nt;
     const double h = 0.5 / p;
-    for (int k = 0; k < (la + 1) * si; ++k) E[k] = 0.0;
-    E[0] = 1.0;
+    E[0] = 1.0;                        // entries with t > i + j are never written and never read
     for (int i = 0; i <= la; ++i) {
         if (i > 0) {
             const double* lo = E + (i - 1) * si;
             double* hi = E + i * si;
             for (int t = 0; t <= i; ++t) {
-                double v = XPA * lo[t];
+                double v = t < i ? XPA * lo[t] : 0.0;
                 if (t > 0) v += h * lo[t - 1];
                 if (t + 1 <= i - 1) v += (double)(t + 1) * lo[t + 1];
                 hi[t] = v;
@@ -106,7 +106,7 @@ __device__ void hermite_table(const int la, const int lb, const double p, const 
             const double* lo = E + i * si + (j - 1) * sj;
             double* hi = E + i * si + j * sj;
             for (int t = 0; t <= i + j; ++t) {
-                double v = XPB * lo[t];
+                double v = t < i + j ? XPB * lo[t] : 0.0;
                 if (t > 0) v += h * lo[t - 1];
                 if (t + 1 <= i + j - 1) v += (double)(t + 1) * lo[t + 1];
                 hi[t] = v;
@@ -114,8 +114,9 @@ __device__ void hermite_table(const int la, const int lb, const double p, const 
         }
     }
     if (alt)
-        for (int k = 0; k < (la + 1) * (lb + 1); ++k)
-            for (int t = 1; t < nt; t += 2) E[k * nt + t] = -E[k * nt + t];
+        for (int i = 0; i <= la; ++i)
+            for (int j = 0; j <= lb; ++j)
+                for (int t = 1; t <= i + j; t += 2) E[i * si + j * sj + t] = -E[i * si + j * sj + t];
 }
 
 // One contracted quartet by the whole CTA.  Results: P[a*sI + b*sJ + c*sK + d] = scale * (ab|cd); with `diag` the
@@ -171,12 +172,13 @@ __device__ void loop_quartet(const int la, const int lb, const int lc, const int
             P[(ab / nb) * sI + (ab % nb) * sJ + (cd / nd) * sK + (cd % nd)] = 0.0;
         }
     }
-    __syncthreads();
+    __syncwarp();
 
     const int npb = (int)bra[3], npk = (int)ket[3];
     for (int ib = 0; ib < npb; ++ib) {
         const double* bp = bra + kPairHeader + ib * kPrimStride;
         const double p = bp[0];
+        bool bra_ready = false;                                    // the bra tables depend on ib only
         for (int ik = 0; ik < npk; ++ik) {
             const double* kp = ket + kPairHeader + ik * kPrimStride;
             const double q = kp[0], pq = p + q;
@@ -184,17 +186,21 @@ __device__ void loop_quartet(const int la, const int lb, const int lc, const int
             if (cut && fabs(pref) < kPrimCut) continue;            // uniform over the CTA
             const double PQx = bp[1] - kp[1], PQy = bp[2] - kp[2], PQz = bp[3] - kp[3];
             const double rho = p * q / pq;
-            if (tid < 3) {
-                hermite_table(la, lb, p, bp[4 + tid], bp[4 + tid] + bra[tid], Eb + tid * o.nEb, false);
-            } else if (tid < 6) {
-                const int x = tid - 3;
-                hermite_table(lc, ld, q, kp[4 + x], kp[4 + x] + ket[x], Ek + x * o.nEk, true);
+            if (tid < 6) {                                         // lanes 0-2: bra x, y, z; lanes 3-5: ket (one call: SIMT)
+                const bool isket = tid >= 3;
+                const int x = isket ? tid - 3 : tid;
+                const double* pr = isket ? kp : bp;
+                const double* hd = isket ? ket : bra;
+                if (isket || !bra_ready)
+                    hermite_table(isket ? lc : la, isket ? ld : lb, isket ? q : p, pr[4 + x], pr[4 + x] + hd[x],
+                                  isket ? Ek + x * o.nEk : Eb + x * o.nEb, isket);
             } else if (tid == 6) {
                 boys_rt(L, rho * (PQx * PQx + PQy * PQy + PQz * PQz), pref, boys, F);
                 double f = 1.0;
                 for (int n = 0; n <= L; ++n) { F[n] *= f; f *= -2.0 * rho; }      // R^n_{000} = (-2 rho)^n F_n
             }
-            __syncthreads();
+            bra_ready = true;
+            __syncwarp();
             // R^n_{tuv} for n = L .. 0; level n needs level n+1 only:  R^n_{t+1,u,v} = t R^{n+1}_{t-1,u,v} + X_PQ R^{n+1}_{tuv}
             for (int n = L; n >= 0; --n) {
                 double* cur = sm + ((n & 1) ? o.R1 : o.R0);
@@ -216,7 +222,7 @@ __device__ void loop_quartet(const int la, const int lb, const int lc, const int
                     }
                     cur[e] = val;
                 }
-                __syncthreads();
+                __syncwarp();
             }
             const double* R = sm + o.R0;
             // H[tuv][cd] = sum_{t'u'v'} (-1)^{t'+u'+v'} E^{cd}_{t'u'v'} R_{t+t',u+u',v+v'}   (sign folded into Ek)
@@ -240,7 +246,7 @@ __device__ void loop_quartet(const int la, const int lb, const int lc, const int
                     }
                 H[e] = s;
             }
-            __syncthreads();
+            __syncwarp();
             // (ab|cd) += sum_{tuv} E^{ab}_{tuv} H[tuv][cd]
             const int nitems = diag ? nab : nab * ncd;
             for (int e = tid; e < nitems; e += kLoopThreads) {
@@ -263,14 +269,14 @@ __device__ void loop_quartet(const int la, const int lb, const int lc, const int
                 if (diag) dg[e] += s;
                 else P[(ab / nb) * sI + (ab % nb) * sJ + (cd / nd) * sK + (cd % nd)] += scale * s;
             }
-            __syncthreads();
+            __syncwarp();
         }
     }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // Panels of one class segment: CTA -> (ket rank r in [ra,rb), shell quartet inside the block quartet).
-__global__ void __launch_bounds__(kLoopThreads) eri_loop_panel_kernel(const EriArgs g, const int la, const int lb,
+__global__ void __launch_bounds__(kLoopThreads, kLoopMinBlocks) eri_loop_panel_kernel(const EriArgs g, const int la, const int lb,
                                                                      const int lc, const int ld)
 {
     extern __shared__ __align__(16) double loop_sm[];
@@ -310,7 +316,7 @@ __global__ void __launch_bounds__(kLoopThreads) eri_loop_panel_kernel(const EriA
                  T.pair_rec + ((size_t)C * T.nshell + D) * T.rec_stride, T.boys, true, scale, P, sI, sJ, sK, false, loop_sm);
 }
 
-__global__ void __launch_bounds__(kLoopThreads) eri_loop_single_kernel(const double* bra, const double* ket,
+__global__ void __launch_bounds__(kLoopThreads, kLoopMinBlocks) eri_loop_single_kernel(const double* bra, const double* ket,
                                                                       const double* boys, const int la, const int lb,
                                                                       const int lc, const int ld, double* out)
 {
@@ -320,7 +326,7 @@ __global__ void __launch_bounds__(kLoopThreads) eri_loop_single_kernel(const dou
 }
 
 // Schwarz bounds of the pair classes with an f shell: Q_AB = sqrt(max_{ab} |(ab|ab)|), one CTA per shell pair.
-__global__ void __launch_bounds__(kLoopThreads) schwarz_loop_kernel(const int nshell, const int a0, const int na,
+__global__ void __launch_bounds__(kLoopThreads, kLoopMinBlocks) schwarz_loop_kernel(const int nshell, const int a0, const int na,
                                                                    const int b0, const int nb,
                                                                    const double* __restrict__ rec, const int rec_stride,
                                                                    const double* __restrict__ boys,
