@@ -7,6 +7,7 @@
 // thread per contracted shell quartet (the paper's mapping; a half-warp for the heaviest classes) and consumed by the
 // digestion kernels (ltjk_digest.cu) before the ring is reused: integrals never form a stored N^4 object.
 // Shell quartets with Q_AB Q_CD < tau (reading A9) are written as zeros.
+#define LTJK_WITH_D1                 // the f-raised generated classes: used here for the six light (f l_b|l_c l_d) classes
 #include "ltjk_internal.h"
 #include "eri_core.h"
 #include "boys_table.h"
@@ -272,7 +273,7 @@ __global__ void __launch_bounds__(kCoopThreads, 1) eri_panel_coop_kernel(const E
     }
 }
 
-static const int kClsLa[kNumPairCls] = {0, 1, 1, 2, 2, 2, 3, 3, 3, 3}, kClsLb[kNumPairCls] = {0, 0, 1, 0, 1, 2, 0, 1, 2, 3};
+static constexpr int kClsLa[kNumPairCls] = {0, 1, 1, 2, 2, 2, 3, 3, 3, 3}, kClsLb[kNumPairCls] = {0, 0, 1, 0, 1, 2, 0, 1, 2, 3};
 
 template <int CB, int CK>
 static int launch_cls(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
@@ -308,6 +309,29 @@ static int launch_cls(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
     }
 }
 
+// Light classes with ONE f shell, (f l_b|l_c l_d) with at most 270 targets: the bulk of the quartets of a basis with few
+// f shells.  gen_eri.py emits straight-line code for them (the f-raised set of the derivative builds), so they run one
+// thread per quartet like the s/p/d classes; every other class with an f shell is looped (ltjk_eri_loop.cu).
+//   bra (fs): ket (ss) (ps) (pp) (ds) (dp);   bra (fp): ket (ss) (ps) (pp) (ds);   bra (fd): ket (ss) (ps)
+inline bool f_class_unrolled(int cb, int ck)
+{
+    return (cb == 6 && ck <= 4) || (cb == 7 && ck <= 3) || (cb == 8 && ck <= 1);
+}
+#define LTJK_F_LIGHT(X) X(0, 0) X(0, 1) X(0, 2) X(0, 3) X(0, 4) X(1, 0) X(1, 1) X(1, 2) X(1, 3) X(2, 0) X(2, 1)
+
+template <int LB, int CK>
+static int launch_f_light(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
+{
+    constexpr int lc[5] = {0, 1, 1, 2, 2}, ld[5] = {0, 0, 1, 0, 1};
+    const long long nthr = (long long)maxkets * g.qn;
+    const int bs = 64;
+    cudaFuncSetAttribute(eri_panel_kernel<3, LB, lc[CK], ld[CK]>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                         cudaSharedmemCarveoutMaxL1);
+    eri_panel_kernel<3, LB, lc[CK], ld[CK]><<<dim3((unsigned)((nthr + bs - 1) / bs), nsub), bs, 0, c->eri_stream>>>(g);
+    LTJK_CUDA(c, cudaGetLastError());
+    return LTJK_OK;
+}
+
 template <int CB>
 static int launch_cls_k(ltjk_ctx* c, int ck, const EriArgs& g, int mk, int ns)
 {
@@ -336,7 +360,14 @@ int launch_eri_panels(ltjk_ctx* c, const Group& gr, int ck)
     g.panel = c->d_panel + (size_t)gr.buf * c->panel_half;
     c->st_launches++;
     const int mk = gr.maxkets[ck], ns = gr.nsub;
-    if (cb >= 6)                                            // a class with an f shell (ck <= cb): looped kernel
+    if (f_class_unrolled(cb, ck)) {
+        switch ((cb - 6) * 6 + ck) {
+#define X(LB, CK) case LB * 6 + CK: return launch_f_light<LB, CK>(c, g, mk, ns);
+            LTJK_F_LIGHT(X)
+#undef X
+        }
+    }
+    if (cb >= 6)                                            // any other class with an f shell (ck <= cb): looped kernel
         return launch_eri_panels_loop(c, g, kClsLa[cb], kClsLb[cb], kClsLa[ck], kClsLb[ck], mk, ns);
     switch (cb) {
     case 0: return launch_cls_k<0>(c, ck, g, mk, ns);
@@ -387,6 +418,15 @@ int launch_eri_single(ltjk_ctx* c, int A, int B, int C, int D, int la, int lb, i
     const int cb = la * (la + 1) / 2 + lb, ck = lc * (lc + 1) / 2 + ld;
     const double* bra = c->t.pair_rec + ((size_t)A * c->nshell + B) * c->t.rec_stride;
     const double* ket = c->t.pair_rec + ((size_t)C * c->nshell + D) * c->t.rec_stride;
+    if (f_class_unrolled(cb, ck) && !looped) {
+        switch ((cb - 6) * 6 + ck) {
+#define X(LB, CK) case LB * 6 + CK: eri_single_kernel<3, LB, kClsLa[CK], kClsLb[CK]><<<1, 32, 0, c->stream>>>(bra, ket, c->t.boys, d_out); break;
+            LTJK_F_LIGHT(X)
+#undef X
+        }
+        LTJK_CUDA(c, cudaGetLastError());
+        return LTJK_OK;
+    }
     if (cb >= 6 || looped) return launch_eri_single_loop(c, bra, ket, la, lb, lc, ld, d_out);
     switch (cb) {
     case 0: single_cls_k<0>(c, ck, bra, ket, d_out); break;
