@@ -177,3 +177,16 @@ def test_jk_in_the_pure_basis_end_to_end(torch_cuda):
     Jr, Kr = O.jk_definition(O.eri_tensor(b), O.cart_from_sph(b, Ds))
     assert relerr(Js.cpu().numpy(), O.sph_from_cart(b, Jr)) < TOL
     assert relerr(Ks.cpu().numpy(), O.sph_from_cart(b, Kr)) < TOL
+
+
+def test_full_size_medium_f_subset_closure(torch_cuda):
+    """400 AO with 10 f shells, the sweep bench.py times under config.f_shells_medium_f (80 densities, production
+    threshold, default panel ring): full N x N matrices of a seeded 8-density subset against the folded oracle O6
+    (about 1.5 min on the 16 host cores of the GPU box), plus the linearity closure over all 80 densities."""
+    from test_gpu_parity import density_subset, full_sweep, linearity_closure
+    w, ctx, Dn, J, K = full_sweep(torch_cuda, "medium_f")
+    assert ctx.get_digest_mode() == 1
+    ds = density_subset(w.nD)
+    Jr, Kr, _ = O.jk_folded(w.basis, Dn[ds].cpu().numpy(), w.schwarz_tau)
+    assert relerr(J[ds].cpu().numpy(), Jr) < TOL and relerr(K[ds].cpu().numpy(), Kr) < TOL
+    linearity_closure(torch_cuda, ctx, Dn, J, K)
