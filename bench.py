@@ -546,6 +546,23 @@ def main():
                                "digest_mode": {1: "block panels", 2: "pair lists"}[repl["digest_mode"]],
                                "transform": repl["transform"]}
         launches += int(repl["launches_per_step"] * 2)
+        # N4: the matrix-level spherical transform of the 192 J matrices (819 MB in, 640 MB out: larger than L2)
+        cl = repl["ctx"]
+        nsl = cl.get_nsph()
+        Jsl = torch.empty((wl.nD, nsl, nsl), dtype=torch.float64, device="cuda")
+        cl.sph_from_cart(repl["J"], Jsl)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(5):
+            cl.sph_from_cart(repl["J"], Jsl)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t_sl = e0.elapsed_time(e1) / 5
+        gbl = 8e-9 * wl.nD * (wl.nao ** 2 + nsl ** 2) / (t_sl * 1e-3)
+        config["large_730"]["sph_from_cart"] = {"n_sph": nsl, "ms": t_sl, "gbs": gbl, "frac_of_hbm_peak": gbl / hbm_peak,
+                                                "bytes": "8 (N^2 + N_sph^2) per matrix, 192 matrices"}
+        launches += 6
+        del Jsl
         repl["ctx"].close()
     out = {"metric": metric_name(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if strong else "weak",

@@ -6,8 +6,9 @@
 //     densities   D^cart[A c, B c'] = sum_{m m'} S^{lA}[m][c] D^sph[A m, B m'] S^{lB}[m'][c']        (S^T D S)
 // S^l = monomial coefficients of the Racah-normalised real solid harmonics, m = -l..l, Cartesian components in the
 // library's lexicographic order; the tables below are written out by hand for l <= 3 (the oracle evaluates the general
-// closed form instead).  Both kernels are plain gather kernels, one thread per output element: HBM-bound
-// (8 (N^2 + N_sph^2) bytes per matrix), the <= 100 multiply-adds per element are hidden behind the loads.
+// closed form instead).  A gather kernel, one thread per output element and one output row per CTA row, so that the
+// row's shell and the (at most 3) non-zero entries of its S row are uniform over the CTA.  Algorithmic traffic
+// 8 (N^2 + N_sph^2) bytes per matrix.
 #include "ltjk_internal.h"
 #include "eri_core.h"
 
@@ -18,7 +19,7 @@ namespace ltjk {
 #define R6 2.449489742783178        /* sqrt 6 */
 #define R10 3.1622776601683795      /* sqrt 10 */
 #define R15 3.872983346207417       /* sqrt 15 */
-__constant__ double kSph[1 + 9 + 30 + 70] = {
+__device__ const double kSph[1 + 9 + 30 + 70] = {       // 880 bytes: stays in L1
     // l = 0
     1.0,
     // l = 1: y, z, x
@@ -53,56 +54,36 @@ struct SphMeta {                 // caller's shell order (the matrices of the C 
     int N, Ns;
 };
 
-// out[n][i][j], i, j pure functions  <-  in[n][mu][nu], Cartesian
-__global__ void __launch_bounds__(256) sph_from_cart_kernel(const SphMeta M, const double* __restrict__ X,
-                                                            double* __restrict__ Y)
+// One CTA row = one output row: blockIdx.y = output row (its shell, and with it the non-zero entries of its S row or
+// column, are uniform over the CTA), threads along the output columns, blockIdx.z = matrix.
+//   DIR 0  out[n][i][j], i, j pure functions  <-  in[n][mu][nu], Cartesian      (operators,  S X S^T)
+//   DIR 1  out[n][mu][nu], Cartesian          <-  in[n][i][j], pure functions   (densities,  S^T D S)
+template <int DIR>
+__global__ void __launch_bounds__(256) sph_row_kernel(const SphMeta M, const double* __restrict__ X, double* __restrict__ Y)
 {
-    __shared__ double S[110];
-    for (int k = threadIdx.x; k < 110; k += blockDim.x) S[k] = kSph[k];
-    __syncthreads();
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= (long long)M.Ns * M.Ns) return;
-    const int i = (int)(e / M.Ns), j = (int)(e % M.Ns);
-    const int A = M.sph_sh[i], B = M.sph_sh[j];
+    const int Nin = DIR == 0 ? M.N : M.Ns, Nout = DIR == 0 ? M.Ns : M.N;
+    const int i = blockIdx.y, j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= Nout) return;
+    const int A = DIR == 0 ? M.sph_sh[i] : M.cart_sh[i], B = DIR == 0 ? M.sph_sh[j] : M.cart_sh[j];
     const int la = M.sh_l[A], lb = M.sh_l[B], na = ncart(la), nb = ncart(lb);
-    const double* Sa = S + sph_tab_off(la) + (i - M.sh_s0[A]) * na;
-    const double* Sb = S + sph_tab_off(lb) + (j - M.sh_s0[B]) * nb;
-    const double* Xn = X + (size_t)blockIdx.y * M.N * M.N + (size_t)M.sh_c0[A] * M.N + M.sh_c0[B];
+    const int ii = i - (DIR == 0 ? M.sh_s0[A] : M.sh_c0[A]), jj = j - (DIR == 0 ? M.sh_s0[B] : M.sh_c0[B]);
+    const int nka = DIR == 0 ? na : 2 * la + 1, nkb = DIR == 0 ? nb : 2 * lb + 1;       // input rows / columns of the shells
+    // S^l[m][c] at m * ncart + c: DIR 0 walks a row (stride 1), DIR 1 a column (stride ncart)
+    const double* Sa = kSph + sph_tab_off(la) + (DIR == 0 ? ii * na : ii);
+    const double* Sb = kSph + sph_tab_off(lb) + (DIR == 0 ? jj * nb : jj);
+    const int sta = DIR == 0 ? 1 : na, stb = DIR == 0 ? 1 : nb;
+    const double* Xn = X + (size_t)blockIdx.z * Nin * Nin + (size_t)(DIR == 0 ? M.sh_c0[A] : M.sh_s0[A]) * Nin +
+                       (DIR == 0 ? M.sh_c0[B] : M.sh_s0[B]);
     double acc = 0.0;
-    for (int ca = 0; ca < na; ++ca) {
-        const double sa = Sa[ca];
-        if (sa == 0.0) continue;
+    for (int ka = 0; ka < nka; ++ka) {
+        const double sa = Sa[ka * sta];
+        if (sa == 0.0) continue;                               // uniform over the CTA: at most 3 rows survive
+        const double* Xr = Xn + (size_t)ka * Nin;
         double row = 0.0;
-        for (int cb = 0; cb < nb; ++cb) row += Sb[cb] * Xn[(size_t)ca * M.N + cb];
+        for (int kb = 0; kb < nkb; ++kb) row += Sb[kb * stb] * Xr[kb];
         acc += sa * row;
     }
-    Y[(size_t)blockIdx.y * M.Ns * M.Ns + e] = acc;
-}
-
-// out[n][mu][nu], Cartesian  <-  in[n][i][j], pure functions
-__global__ void __launch_bounds__(256) cart_from_sph_kernel(const SphMeta M, const double* __restrict__ D,
-                                                            double* __restrict__ Y)
-{
-    __shared__ double S[110];
-    for (int k = threadIdx.x; k < 110; k += blockDim.x) S[k] = kSph[k];
-    __syncthreads();
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= (long long)M.N * M.N) return;
-    const int mu = (int)(e / M.N), nu = (int)(e % M.N);
-    const int A = M.cart_sh[mu], B = M.cart_sh[nu];
-    const int la = M.sh_l[A], lb = M.sh_l[B], na = ncart(la), nb = ncart(lb);
-    const double* Sa = S + sph_tab_off(la) + (mu - M.sh_c0[A]);        // column ca of S^{la}: stride na
-    const double* Sb = S + sph_tab_off(lb) + (nu - M.sh_c0[B]);
-    const double* Dn = D + (size_t)blockIdx.y * M.Ns * M.Ns + (size_t)M.sh_s0[A] * M.Ns + M.sh_s0[B];
-    double acc = 0.0;
-    for (int ma = 0; ma < 2 * la + 1; ++ma) {
-        const double sa = Sa[ma * na];
-        if (sa == 0.0) continue;
-        double row = 0.0;
-        for (int mb = 0; mb < 2 * lb + 1; ++mb) row += Sb[mb * nb] * Dn[(size_t)ma * M.Ns + mb];
-        acc += sa * row;
-    }
-    Y[(size_t)blockIdx.y * M.N * M.N + e] = acc;
+    Y[(size_t)blockIdx.z * Nout * Nout + (size_t)i * Nout + j] = acc;
 }
 
 void free_sph(ltjk_ctx* c)
@@ -154,13 +135,12 @@ int ltjk_sph_from_cart(ltjk_ctx* c, int nmat, const double* X_cart, double* X_sp
 {
     if (!c) return LTJK_EINVAL;
     if (!c->have_basis) return set_err(c, LTJK_ENOBASIS, "sph_from_cart: no basis");
-    if (nmat <= 0 || nmat > 65535 || !X_cart || !X_sph) return set_err(c, LTJK_EINVAL, "sph_from_cart: bad arguments (1 <= nmat <= 65535)");
+    if (nmat <= 0 || nmat > 65535 || c->nao > 65535 || !X_cart || !X_sph) return set_err(c, LTJK_EINVAL, "sph_from_cart: bad arguments (1 <= nmat <= 65535)");
     cudaSetDevice(c->device);
     SphMeta M;
     int rc;
     if ((rc = ensure_sph(c, &M))) return rc;
-    const long long n = (long long)M.Ns * M.Ns;
-    sph_from_cart_kernel<<<dim3((unsigned)((n + 255) / 256), nmat), 256, 0, c->stream>>>(M, X_cart, X_sph);
+    sph_row_kernel<0><<<dim3((M.Ns + 255) / 256, M.Ns, nmat), 256, 0, c->stream>>>(M, X_cart, X_sph);
     LTJK_CUDA(c, cudaGetLastError());
     return LTJK_OK;
 }
@@ -169,13 +149,12 @@ int ltjk_cart_from_sph(ltjk_ctx* c, int nmat, const double* D_sph, double* D_car
 {
     if (!c) return LTJK_EINVAL;
     if (!c->have_basis) return set_err(c, LTJK_ENOBASIS, "cart_from_sph: no basis");
-    if (nmat <= 0 || nmat > 65535 || !D_sph || !D_cart) return set_err(c, LTJK_EINVAL, "cart_from_sph: bad arguments (1 <= nmat <= 65535)");
+    if (nmat <= 0 || nmat > 65535 || c->nao > 65535 || !D_sph || !D_cart) return set_err(c, LTJK_EINVAL, "cart_from_sph: bad arguments (1 <= nmat <= 65535)");
     cudaSetDevice(c->device);
     SphMeta M;
     int rc;
     if ((rc = ensure_sph(c, &M))) return rc;
-    const long long n = (long long)M.N * M.N;
-    cart_from_sph_kernel<<<dim3((unsigned)((n + 255) / 256), nmat), 256, 0, c->stream>>>(M, D_sph, D_cart);
+    sph_row_kernel<1><<<dim3((M.N + 255) / 256, M.N, nmat), 256, 0, c->stream>>>(M, D_sph, D_cart);
     LTJK_CUDA(c, cudaGetLastError());
     return LTJK_OK;
 }
