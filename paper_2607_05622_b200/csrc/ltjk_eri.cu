@@ -318,6 +318,28 @@ inline bool f_class_unrolled(int cb, int ck)
     return (cb == 6 && ck <= 4) || (cb == 7 && ck <= 3) || (cb == 8 && ck <= 1);
 }
 #define LTJK_F_LIGHT(X) X(0, 0) X(0, 1) X(0, 2) X(0, 3) X(0, 4) X(1, 0) X(1, 1) X(1, 2) X(1, 3) X(2, 0) X(2, 1)
+// Four heavier one-f classes with l_b, l_d > 0 -- (fp|dp), (fp|dd), (fd|pp), (fd|dp): 540-1080 targets -- go through the
+// cooperative kernel (a half-warp per quartet, contracted targets in shared memory) like (dd|dd).
+inline bool f_class_coop(int cb, int ck) { return (cb == 7 && (ck == 4 || ck == 5)) || (cb == 8 && (ck == 2 || ck == 4)); }
+#define LTJK_F_COOP(X) X(1, 4) X(1, 5) X(2, 2) X(2, 4)
+
+template <int LB, int CK>
+static int launch_f_coop(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
+{
+    constexpr int lc[6] = {0, 1, 1, 2, 2, 2}, ld[6] = {0, 0, 1, 0, 1, 2};
+    using V = ltjk_gen::Vrr<3, LB, lc[CK], ld[CK]>;
+    constexpr int QS = V::NE * V::NF + ltjk_gen::Hrr<3, LB>::NAB * V::NF;
+    constexpr int smem = (kCoopThreads / 16) * QS * (int)sizeof(double);
+    static_assert(smem <= 227 * 1024, "cooperative ERI kernel: shared memory");
+    LTJK_CUDA(c, cudaFuncSetAttribute(eri_panel_coop_kernel<3, LB, lc[CK], ld[CK]>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    const long long nq = (long long)maxkets * g.qn;
+    const int per = kCoopThreads / 16;
+    eri_panel_coop_kernel<3, LB, lc[CK], ld[CK]>
+        <<<dim3((unsigned)((nq + per - 1) / per), nsub), kCoopThreads, smem, c->eri_stream>>>(g);
+    LTJK_CUDA(c, cudaGetLastError());
+    return LTJK_OK;
+}
 
 template <int LB, int CK>
 static int launch_f_light(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
@@ -364,6 +386,13 @@ int launch_eri_panels(ltjk_ctx* c, const Group& gr, int ck)
         switch ((cb - 6) * 6 + ck) {
 #define X(LB, CK) case LB * 6 + CK: return launch_f_light<LB, CK>(c, g, mk, ns);
             LTJK_F_LIGHT(X)
+#undef X
+        }
+    }
+    if (f_class_coop(cb, ck)) {
+        switch ((cb - 6) * 6 + ck) {
+#define X(LB, CK) case LB * 6 + CK: return launch_f_coop<LB, CK>(c, g, mk, ns);
+            LTJK_F_COOP(X)
 #undef X
         }
     }
