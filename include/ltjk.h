@@ -54,8 +54,9 @@ int ltjk_set_scratch_bytes(ltjk_ctx* ctx, long long bytes);
 /* Basis upload (step a1).  HOST pointers, copied.
  *   xyz[natom*3]        centres, bohr
  *   atom[nshell]        centre index of each shell
- *   l[nshell]           angular momentum, 0..3 (else LTJK_ELMAX).  s, p, d classes run generated straight-line code; every
- *                       class with an f shell runs the looped kernel (PAPER.md:L316 two codegen regimes).
+ *   l[nshell]           angular momentum, 0..3 (else LTJK_ELMAX).  s, p, d classes and the lighter classes with one f shell
+ *                       run generated straight-line code, the other classes with an f shell the looped kernel
+ *                       (PAPER.md:L316 two codegen regimes).
  *                       Cartesian components in lexicographic order (f: xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz)
  *   nprim[nshell]       primitives per shell, 1..4
  *   prim_off[nshell]    first primitive of the shell in exps/coef
@@ -229,9 +230,9 @@ int ltjk_debug_poison(ltjk_ctx* ctx, int enable);
  * device ERI kernel, written to HOST out[na*nb*nc*nd] (row-major a,b,c,d).  Synchronises. */
 int ltjk_debug_eri_quartet(ltjk_ctx* ctx, int A, int B, int C, int D, double* out_host);
 
-/* Test hook: the same quartet through the LOOPED evaluation (csrc/ltjk_eri_loop.cu) whatever its class.  Classes with an
- * f shell always take that path; for s, p, d classes this is the cross-check PAPER.md:L316 states for its two codegen
- * regimes ("machine-epsilon equal to the unrolled path").  Synchronises. */
+/* Test hook: the same quartet through the LOOPED evaluation (csrc/ltjk_eri_loop.cu) whatever its class.  Classes with
+ * two or more f shells always take that path; for the classes with generated code this is the cross-check PAPER.md:L316
+ * states for its two codegen regimes ("machine-epsilon equal to the unrolled path").  Synchronises. */
 int ltjk_debug_eri_quartet_looped(ltjk_ctx* ctx, int A, int B, int C, int D, double* out_host);
 
 /* Test hook: device Boys function F_m(T), m = 0..mmax (mmax <= 8), for n arguments T_host[n];
