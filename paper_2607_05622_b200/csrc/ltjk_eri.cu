@@ -309,15 +309,16 @@ static int launch_cls(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
     }
 }
 
-// Light classes with ONE f shell, (f l_b|l_c l_d) with at most 270 targets: the bulk of the quartets of a basis with few
+// Light classes with ONE f shell, (f l_b|l_c l_d) with at most 360 targets: the bulk of the quartets of a basis with few
 // f shells.  gen_eri.py emits straight-line code for them (the f-raised set of the derivative builds), so they run one
-// thread per quartet like the s/p/d classes; every other class with an f shell is looped (ltjk_eri_loop.cu).
-//   bra (fs): ket (ss) (ps) (pp) (ds) (dp);   bra (fp): ket (ss) (ps) (pp) (ds);   bra (fd): ket (ss) (ps)
+// thread per quartet like the s/p/d classes; every class with an f shell that is neither here nor in the cooperative
+// set below is looped (ltjk_eri_loop.cu).
+//   bra (fs): every ket (ss) ... (dd);   bra (fp): ket (ss) (ps) (pp) (ds);   bra (fd): ket (ss) (ps) (ds)
 inline bool f_class_unrolled(int cb, int ck)
 {
-    return (cb == 6 && ck <= 4) || (cb == 7 && ck <= 3) || (cb == 8 && ck <= 1);
+    return (cb == 6 && ck <= 5) || (cb == 7 && ck <= 3) || (cb == 8 && (ck <= 1 || ck == 3));
 }
-#define LTJK_F_LIGHT(X) X(0, 0) X(0, 1) X(0, 2) X(0, 3) X(0, 4) X(1, 0) X(1, 1) X(1, 2) X(1, 3) X(2, 0) X(2, 1)
+#define LTJK_F_LIGHT(X) X(0, 0) X(0, 1) X(0, 2) X(0, 3) X(0, 4) X(0, 5) X(1, 0) X(1, 1) X(1, 2) X(1, 3) X(2, 0) X(2, 1) X(2, 3)
 // Four heavier one-f classes with l_b, l_d > 0 -- (fp|dp), (fp|dd), (fd|pp), (fd|dp): 540-1080 targets -- go through the
 // cooperative kernel (a half-warp per quartet, contracted targets in shared memory) like (dd|dd).
 inline bool f_class_coop(int cb, int ck) { return (cb == 7 && (ck == 4 || ck == 5)) || (cb == 8 && (ck == 2 || ck == 4)); }
@@ -344,7 +345,7 @@ static int launch_f_coop(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
 template <int LB, int CK>
 static int launch_f_light(ltjk_ctx* c, const EriArgs& g, int maxkets, int nsub)
 {
-    constexpr int lc[5] = {0, 1, 1, 2, 2}, ld[5] = {0, 0, 1, 0, 1};
+    constexpr int lc[6] = {0, 1, 1, 2, 2, 2}, ld[6] = {0, 0, 1, 0, 1, 2};
     const long long nthr = (long long)maxkets * g.qn;
     const int bs = 64;
     cudaFuncSetAttribute(eri_panel_kernel<3, LB, lc[CK], ld[CK]>, cudaFuncAttributePreferredSharedMemoryCarveout,

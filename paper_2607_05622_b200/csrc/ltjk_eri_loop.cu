@@ -2,7 +2,7 @@
 //
 // "For f shells and above the kernel is instead looped: the ladder structure ... is encoded as integer
 // index tables walked by runtime loops, so source size is O(tables) rather than O(nodes)".  The straight-line generated
-// code of csrc/gen/ stops at (dd|dd) plus the one-f classes of the derivative builds, 15 of which the value builds use
+// code of csrc/gen/ stops at (dd|dd) plus the one-f classes of the derivative builds, 17 of which the value builds use
 // (ltjk_eri.cu); every other class with an l = 3 shell comes here.  Angular momenta are run-time
 // arguments, the recurrences are loops over small index tables built in shared memory, and -- unlike the paper's
 // one-thread-per-quartet mapping, whose per-thread working set ((ff|ff): 10^4 outputs) only fits an HBM scratch slab
