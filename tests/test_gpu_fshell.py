@@ -25,8 +25,8 @@ def four_centre_basis(lmax):
 
 def test_eri_f_classes_vs_oracle(torch_cuda):
     """All 175 ordered classes (la lb|lc ld), l <= 3, with at least one f shell, two-primitive contractions, against the
-    oracle: through the path the builds take (generated straight-line code for the six light classes (f s|..), (f p|..)
-    with ket (ss), (ps), (pp); the looped kernel for the rest) and through the looped kernel for every class."""
+    oracle: through the path the hook takes by default (generated straight-line code where the library uses it for the
+    builds' per-thread one-f classes, the looped kernel for the rest) and through the looped kernel for every class."""
     b = four_centre_basis(3)
     ctx = make_ctx(b)
     worst = 0.0
@@ -35,7 +35,7 @@ def test_eri_f_classes_vs_oracle(torch_cuda):
             continue
         A, B, C, D = (4 * i + l for i, l in enumerate(ls))
         ref = O.eri_shell(b, A, B, C, D)
-        for looped in (False, True):       # False: the path the builds take (six light classes are unrolled); True: looped
+        for looped in (False, True):       # False: generated code where the per-thread builds use it; True: looped
             out = ctx.debug_eri_quartet(b, A, B, C, D, looped=looped)
             err = np.abs(out - ref).max() / np.abs(ref).max()
             worst = max(worst, err)
