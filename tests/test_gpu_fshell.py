@@ -190,3 +190,38 @@ def test_full_size_medium_f_subset_closure(torch_cuda):
     Jr, Kr, _ = O.jk_folded(w.basis, Dn[ds].cpu().numpy(), w.schwarz_tau)
     assert relerr(J[ds].cpu().numpy(), Jr) < TOL and relerr(K[ds].cpu().numpy(), Kr) < TOL
     linearity_closure(torch_cuda, ctx, Dn, J, K)
+
+
+def test_f_shells_with_resident_panels_sharding_and_poison(torch_cuda):
+    """The other modes of the block-panel path do not know which kernel wrote a panel: resident panels reused by a
+    second build, a build split over three ranks in quartet space, and the NaN write-coverage hook (every panel element
+    the digestion reads was written by a per-thread, cooperative or looped ERI kernel, or by the zero fill), all on
+    the s/p/d/f basis with a small ring."""
+    from paper_2607_05622_b200 import ltjk
+    torch = torch_cuda
+    b = spdf_basis()
+    D = random_densities(b.nao, 6, seed=23)
+    Jr, Kr = O.jk_definition(O.eri_tensor(b), D)
+    # resident panels
+    ctx = ltjk.Context(0)
+    ctx.set_resident(True)
+    ctx.set_basis(b)
+    ctx.build_shell_pairs(0.0)
+    J1, K1 = gpu_jk(torch, ctx, D[:2])
+    n_first = ctx.get_stats()["n_launches"]
+    J2, K2 = gpu_jk(torch, ctx, D)
+    assert ctx.get_stats()["n_launches"] < n_first              # no ERI launches in the second build
+    assert relerr(J1, Jr[:2]) < TOL and relerr(K1, Kr[:2]) < TOL
+    assert relerr(J2, Jr) < TOL and relerr(K2, Kr) < TOL
+    ctx.close()
+    # quartet sharding + poisoned ring
+    ctx = make_ctx(b, tau=0.0, scratch=1 << 20)
+    ctx.debug_poison(True)
+    Jsum, Ksum = np.zeros_like(D), np.zeros_like(D)
+    for r in range(3):
+        ctx.set_quartet_shard(r, 3)
+        Jp, Kp = gpu_jk(torch, ctx, D)
+        assert np.isfinite(Jp).all() and np.isfinite(Kp).all() and np.abs(Kp).max() > 0
+        Jsum += Jp
+        Ksum += Kp
+    assert relerr(Jsum, Jr) < TOL and relerr(Ksum, Kr) < TOL
